@@ -1,0 +1,108 @@
+"""CPU oracle for the H-ADPSGD super-learner step -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Thin ctypes/numpy wrapper over ``libhadpsgd_oracle.so`` (plain single-threaded C++,
+``oracle/hadpsgd_oracle.cpp``, written from PAPER.md).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It imports nothing from
+``paper_1907_05701_b200`` and the product imports nothing from here.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+GRAD_F32 = 0
+GRAD_BF16 = 1
+NO_MIX = 1 << 0
+EQ7_LITERAL = 1 << 1
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        from . import build as _build  # lazy: keeps `python -m oracle.build` clean
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        i32, i64, u64, u32 = ctypes.c_int, ctypes.c_int64, ctypes.c_uint64, ctypes.c_uint32
+        vp, f32, f64 = ctypes.c_void_p, ctypes.c_float, ctypes.c_double
+        L.hadpsgd_oracle_partner.argtypes = [i32, u64, vp]
+        L.hadpsgd_oracle_mixing_matrix.argtypes = [i32, u64, vp]
+        L.hadpsgd_oracle_step.argtypes = [i32, i32, i64, vp, i32, vp, vp, f32, f32, u64, u32, vp]
+        L.hadpsgd_oracle_step_f64.argtypes = [i32, i32, i64, vp, i32, vp, vp, f64, f64, u64, u32]
+        L.hadpsgd_oracle_consensus_distance.argtypes = [i32, i64, vp, vp]
+        for fn in (L.hadpsgd_oracle_partner, L.hadpsgd_oracle_mixing_matrix, L.hadpsgd_oracle_step,
+                   L.hadpsgd_oracle_step_f64, L.hadpsgd_oracle_consensus_distance):
+            fn.restype = i32
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def partner(S, step_k):
+    out = np.empty(S, dtype=np.int32)
+    rc = lib().hadpsgd_oracle_partner(S, step_k, _ptr(out))
+    if rc != 0:
+        raise ValueError(f"hadpsgd_oracle_partner(S={S}) rc={rc}")
+    return out
+
+
+def mixing_matrix(S, step_k):
+    T = np.empty((S, S), dtype=np.float64)
+    rc = lib().hadpsgd_oracle_mixing_matrix(S, step_k, _ptr(T))
+    if rc != 0:
+        raise ValueError(f"hadpsgd_oracle_mixing_matrix(S={S}) rc={rc}")
+    return T
+
+
+def _check(grads, w, v, wdtype):
+    assert grads.ndim == 3 and grads.flags.c_contiguous
+    S, G, P = grads.shape
+    if grads.dtype == np.float32:
+        gd = GRAD_F32
+    elif grads.dtype == np.uint16:  # bf16 bit patterns
+        gd = GRAD_BF16
+    else:
+        raise TypeError("grads must be float32 or uint16 (bf16 bits)")
+    for a in (w, v):
+        assert a.dtype == wdtype and a.shape == (S, P) and a.flags.c_contiguous and a.flags.writeable
+    return S, G, P, gd
+
+
+def step(grads, w, v, lr, mu, step_k, flags=0, diag=False):
+    """In-place fp32 step on w, v (numpy float32 [S,P]); grads [S,G,P] float32 or uint16(bf16).
+
+    Returns None, or a dict of double arrays gsq[S], wsq[S], gap[S] when diag=True."""
+    S, G, P, gd = _check(grads, w, v, np.float32)
+    d = np.zeros(3 * S, dtype=np.float64) if diag else None
+    rc = lib().hadpsgd_oracle_step(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
+                                   float(lr), float(mu), int(step_k), int(flags),
+                                   _ptr(d) if diag else None)
+    if rc != 0:
+        raise ValueError(f"hadpsgd_oracle_step rc={rc}")
+    if diag:
+        return {"gsq": d[:S].copy(), "wsq": d[S:2 * S].copy(), "gap": d[2 * S:].copy()}
+    return None
+
+
+def step_f64(grads, w, v, lr, mu, step_k, flags=0):
+    """In-place double-precision shadow step on w, v (numpy float64 [S,P])."""
+    S, G, P, gd = _check(grads, w, v, np.float64)
+    rc = lib().hadpsgd_oracle_step_f64(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
+                                       float(lr), float(mu), int(step_k), int(flags))
+    if rc != 0:
+        raise ValueError(f"hadpsgd_oracle_step_f64 rc={rc}")
+
+
+def consensus_distance(w):
+    assert w.dtype == np.float32 and w.ndim == 2 and w.flags.c_contiguous
+    out = np.zeros(1, dtype=np.float64)
+    rc = lib().hadpsgd_oracle_consensus_distance(w.shape[0], w.shape[1], _ptr(w), _ptr(out))
+    if rc != 0:
+        raise ValueError("hadpsgd_oracle_consensus_distance failed")
+    return float(out[0])

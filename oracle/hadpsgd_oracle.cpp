@@ -1,0 +1,207 @@
+// hadpsgd_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see hadpsgd_oracle.h).
+//
+// Single thread, no blocking, no fusion, no reordering: the loops below are the
+// algorithm of DESIGN.md section 3 in the paper's order so a reader can check
+// them against PAPER.md by eye.  Build: g++ -O2 -ffp-contract=off -fno-fast-math
+// (oracle/build.py) -- -ffp-contract=off is REQUIRED so that a*b+c is two
+// roundings, which is what the deterministic CUDA mode must match bit for bit.
+//
+// No CUDA header, no header from paper_1907_05701_b200/, nothing shared.
+
+#include "hadpsgd_oracle.h"
+
+#include <cstring>
+#include <vector>
+
+namespace {
+
+// bf16 -> fp32 is exact: a bf16 value is the top 16 bits of an fp32 (R6).
+inline float widen_bf16(uint16_t h) {
+    uint32_t bits = static_cast<uint32_t>(h) << 16;
+    float f;
+    std::memcpy(&f, &bits, sizeof f);
+    return f;
+}
+
+inline float load_grad(const void* grads, int grad_dtype, int64_t idx) {
+    if (grad_dtype == ORACLE_GRAD_BF16) return widen_bf16(static_cast<const uint16_t*>(grads)[idx]);
+    return static_cast<const float*>(grads)[idx];
+}
+
+bool build_partner(int S, uint64_t step_k, uint32_t flags, std::vector<int32_t>& partner) {
+    if (S < 1) return false;
+    partner.resize(S);
+    if (S == 1 || (flags & ORACLE_NO_MIX)) {
+        for (int s = 0; s < S; ++s) partner[s] = s;
+        return true;
+    }
+    if (S % 2 != 0) return false;  // R8: no perfect matching => T_k of PAPER.md:66 does not exist
+    if (step_k % 2 == 0) {
+        for (int i = 0; i < S / 2; ++i) {  // (2i, 2i+1)
+            partner[2 * i] = 2 * i + 1;
+            partner[2 * i + 1] = 2 * i;
+        }
+    } else {
+        for (int i = 0; i < S / 2; ++i) {  // (2i+1, (2i+2) mod S)
+            int a = 2 * i + 1, b = (2 * i + 2) % S;
+            partner[a] = b;
+            partner[b] = a;
+        }
+    }
+    return true;
+}
+
+}  // namespace
+
+extern "C" int hadpsgd_oracle_partner(int S, uint64_t step_k, int32_t* partner) {
+    if (!partner) return -1;
+    std::vector<int32_t> p;
+    if (!build_partner(S, step_k, 0, p)) return -1;
+    for (int s = 0; s < S; ++s) partner[s] = p[s];
+    return 0;
+}
+
+extern "C" int hadpsgd_oracle_mixing_matrix(int S, uint64_t step_k, double* T) {
+    if (!T) return -1;
+    std::vector<int32_t> p;
+    if (!build_partner(S, step_k, 0, p)) return -1;
+    for (int64_t k = 0; k < static_cast<int64_t>(S) * S; ++k) T[k] = 0.0;
+    for (int s = 0; s < S; ++s) {
+        if (p[s] == s) {
+            T[static_cast<int64_t>(s) * S + s] = 1.0;
+        } else {
+            T[static_cast<int64_t>(s) * S + s] = 0.5;
+            T[static_cast<int64_t>(s) * S + p[s]] = 0.5;
+        }
+    }
+    return 0;
+}
+
+extern "C" int hadpsgd_oracle_step(int S, int G, int64_t P, const void* grads, int grad_dtype,
+                                   float* w, float* v, float lr, float mu, uint64_t step_k,
+                                   uint32_t flags, double* diag) {
+    if (S < 1 || G < 1 || P < 0 || !grads || !w || !v) return -1;
+    if (grad_dtype != ORACLE_GRAD_F32 && grad_dtype != ORACLE_GRAD_BF16) return -1;
+    std::vector<int32_t> partner;
+    if (!build_partner(S, step_k, flags, partner)) return -1;
+
+    const float invG = 1.0f / static_cast<float>(G);  // R5: mean = fp32 sum * fp32 reciprocal
+    std::vector<float> u(static_cast<size_t>(S) * static_cast<size_t>(P));
+    double* gsq = diag ? diag : nullptr;
+    double* wsq = diag ? diag + S : nullptr;
+    double* gap = diag ? diag + 2 * S : nullptr;
+    if (diag)
+        for (int k = 0; k < 3 * S; ++k) diag[k] = 0.0;
+
+    // phase 1: intra-super-learner mean (eq. (6)), momentum SGD (eq. (3) + R2)
+    for (int s = 0; s < S; ++s) {
+        for (int64_t i = 0; i < P; ++i) {
+            float acc = load_grad(grads, grad_dtype, (static_cast<int64_t>(s) * G + 0) * P + i);
+            for (int g = 1; g < G; ++g)
+                acc = acc + load_grad(grads, grad_dtype, (static_cast<int64_t>(s) * G + g) * P + i);
+            float gbar = acc * invG;
+            float t = mu * v[s * P + i];
+            float vnew = t + gbar;
+            v[s * P + i] = vnew;
+            float t2 = lr * vnew;
+            if (flags & ORACLE_EQ7_LITERAL)
+                u[s * P + i] = t2;  // kept aside: subtracted AFTER mixing the old weights
+            else
+                u[s * P + i] = w[s * P + i] - t2;
+            if (diag) gsq[s] += static_cast<double>(gbar) * static_cast<double>(gbar);
+        }
+    }
+
+    // phase 2: pairwise averaging with the ring neighbour (eq. (7), T_k)
+    for (int s = 0; s < S; ++s) {
+        int p = partner[s];
+        if (p < s) continue;  // each pair once; p == s means unpaired
+        for (int64_t i = 0; i < P; ++i) {
+            if (flags & ORACLE_EQ7_LITERAL) {
+                // Theta_{k+1} = Theta_k T_k - alpha g : mix OLD weights, subtract own update
+                float ws = w[s * P + i], wp = w[p * P + i];
+                float m = (p == s) ? ws : 0.5f * (ws + wp);
+                if (diag) {
+                    double d = static_cast<double>(ws) - static_cast<double>(wp);
+                    gap[s] += d * d;
+                }
+                w[s * P + i] = m - u[s * P + i];
+                if (p != s) w[p * P + i] = m - u[p * P + i];
+            } else {
+                float us = u[s * P + i], up = u[p * P + i];
+                float m = (p == s) ? us : 0.5f * (us + up);
+                if (diag) {
+                    double d = static_cast<double>(us) - static_cast<double>(up);
+                    gap[s] += d * d;
+                }
+                w[s * P + i] = m;
+                if (p != s) w[p * P + i] = m;
+            }
+            if (diag) {
+                wsq[s] += static_cast<double>(w[s * P + i]) * static_cast<double>(w[s * P + i]);
+                if (p != s)
+                    wsq[p] += static_cast<double>(w[p * P + i]) * static_cast<double>(w[p * P + i]);
+            }
+        }
+        if (diag && p != s) gap[p] = gap[s];
+    }
+    return 0;
+}
+
+extern "C" int hadpsgd_oracle_step_f64(int S, int G, int64_t P, const void* grads, int grad_dtype,
+                                       double* w, double* v, double lr, double mu,
+                                       uint64_t step_k, uint32_t flags) {
+    if (S < 1 || G < 1 || P < 0 || !grads || !w || !v) return -1;
+    if (grad_dtype != ORACLE_GRAD_F32 && grad_dtype != ORACLE_GRAD_BF16) return -1;
+    std::vector<int32_t> partner;
+    if (!build_partner(S, step_k, flags, partner)) return -1;
+
+    std::vector<double> u(static_cast<size_t>(S) * static_cast<size_t>(P));
+    for (int s = 0; s < S; ++s) {
+        for (int64_t i = 0; i < P; ++i) {
+            double acc = 0.0;
+            for (int g = 0; g < G; ++g)
+                acc += static_cast<double>(
+                    load_grad(grads, grad_dtype, (static_cast<int64_t>(s) * G + g) * P + i));
+            double gbar = acc / static_cast<double>(G);
+            double vnew = mu * v[s * P + i] + gbar;
+            v[s * P + i] = vnew;
+            if (flags & ORACLE_EQ7_LITERAL)
+                u[s * P + i] = lr * vnew;
+            else
+                u[s * P + i] = w[s * P + i] - lr * vnew;
+        }
+    }
+    for (int s = 0; s < S; ++s) {
+        int p = partner[s];
+        if (p < s) continue;
+        for (int64_t i = 0; i < P; ++i) {
+            if (flags & ORACLE_EQ7_LITERAL) {
+                double m = (p == s) ? w[s * P + i] : 0.5 * (w[s * P + i] + w[p * P + i]);
+                w[s * P + i] = m - u[s * P + i];
+                if (p != s) w[p * P + i] = m - u[p * P + i];
+            } else {
+                double m = (p == s) ? u[s * P + i] : 0.5 * (u[s * P + i] + u[p * P + i]);
+                w[s * P + i] = m;
+                if (p != s) w[p * P + i] = m;
+            }
+        }
+    }
+    return 0;
+}
+
+extern "C" int hadpsgd_oracle_consensus_distance(int S, int64_t P, const float* w, double* out) {
+    if (S < 1 || P < 0 || !w || !out) return -1;
+    double D = 0.0;
+    for (int64_t i = 0; i < P; ++i) {
+        double mean = 0.0;
+        for (int s = 0; s < S; ++s) mean += static_cast<double>(w[s * P + i]);
+        mean /= static_cast<double>(S);
+        for (int s = 0; s < S; ++s) {
+            double d = static_cast<double>(w[s * P + i]) - mean;
+            D += d * d;
+        }
+    }
+    *out = D;
+    return 0;
+}

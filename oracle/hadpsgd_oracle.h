@@ -1,0 +1,83 @@
+/*
+ * hadpsgd_oracle.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded CPU definition of one H-ADPSGD super-learner
+ * step, written from /root/reference/PAPER.md (arxiv 1907.05701) and the
+ * readings listed in DESIGN.md section 3.  It shares no code, header, table or
+ * helper with the CUDA path under paper_1907_05701_b200/.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load it.
+ *
+ * Every function here is pinned by tests/test_oracle_pins.py against closed
+ * forms, exact-rational arithmetic, brute-force dense mixing matrices and the
+ * invariants the paper states; no function is "parity unpinned".
+ *
+ * All pointers are HOST pointers.  Layout is row-major:
+ *     grads[s][g][i]  (S*G*P elements; fp32, or bf16 stored as uint16)
+ *     w[s][i], v[s][i] (S*P fp32, or S*P fp64 for the _f64 shadow)
+ * Return value: 0 = ok, -1 = invalid argument.
+ */
+#ifndef HADPSGD_ORACLE_H
+#define HADPSGD_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORACLE_GRAD_F32 = 0, ORACLE_GRAD_BF16 = 1 };
+
+/* flags */
+enum {
+    ORACLE_NO_MIX       = 1u << 0, /* T_k = I : every super-learner keeps u_s (eq. (6)/(3) only)     */
+    ORACLE_EQ7_LITERAL  = 1u << 1  /* eq. (7) as printed: w'_s = 1/2 (w_s + w_p) - lr * v_s           */
+};
+
+/* Pairing (reading R7; "left or right neighbor in the
+ * ring"): even step_k pairs (2i, 2i+1); odd step_k pairs (2i+1, (2i+2) mod S).
+ * S == 1 -> partner[0] = 0.  S odd and > 1 -> -1 (no perfect matching, R8).   */
+int hadpsgd_oracle_partner(int S, uint64_t step_k, int32_t* partner /*[S]*/);
+
+/* Dense mixing matrix T_k (symmetric, doubly stochastic, two 0.5
+ * per row and column).  With the update-then-average reading (R3) a pair
+ * (s,p) contributes T[s][s]=T[s][p]=T[p][s]=T[p][p]=0.5.  Row-major S x S.   */
+int hadpsgd_oracle_mixing_matrix(int S, uint64_t step_k, double* T /*[S*S]*/);
+
+/* One step, fp32 storage and fp32 arithmetic, one rounding per operation, no
+ * FMA contraction (compiled -ffp-contract=off), fixed left-to-right learner
+ * order.  This is the bit pattern the CUDA path must reproduce in its
+ * deterministic mode.
+ *   phase 1 (eq. (6) PAPER.md:57 then eq. (3) PAPER.md:34 + momentum, R2):
+ *       acc  = grads[s][0][i] + grads[s][1][i] + ... (left to right)
+ *       gbar = acc * (1.0f/G)
+ *       v    = mu*v + gbar          (mul, then add)
+ *       u    = w - lr*v             (mul, then sub)
+ *   phase 2 (eq. (7), T_k PAPER.md:66, order per PAPER.md:62, R3):
+ *       w_s = w_p = 0.5f * (u_s + u_p)
+ * diag (optional, may be NULL): doubles laid out
+ *       gsq[S] | wsq[S] | gap[S]   (gap[s] == gap[partner[s]]; 0 if unpaired)
+ *   gsq[s] = sum_i gbar^2, wsq[s] = sum_i w'^2, gap[s] = sum_i (u_s-u_p)^2,
+ *   each term formed in double from the fp32 values.
+ * grads are read-only; w and v are updated in place.                          */
+int hadpsgd_oracle_step(int S, int G, int64_t P,
+                        const void* grads, int grad_dtype,
+                        float* w, float* v,
+                        float lr, float mu, uint64_t step_k, uint32_t flags,
+                        double* diag /* [3*S] or NULL */);
+
+/* The same algorithm carried in double (state in double, gradients widened
+ * exactly).  Used by the closed-form pins and to derive the fp32 tolerance.  */
+int hadpsgd_oracle_step_f64(int S, int G, int64_t P,
+                            const void* grads, int grad_dtype,
+                            double* w, double* v,
+                            double lr, double mu, uint64_t step_k, uint32_t flags);
+
+/* Consensus distance D = sum_s sum_i (w[s][i] - mean_s w[.][i])^2 in double
+ * (repeated mixing drives all learners to (1/n) sum theta^i).   */
+int hadpsgd_oracle_consensus_distance(int S, int64_t P, const float* w, double* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,406 @@
+"""Pins for the CPU oracle (oracle/) against what the paper and the mathematics fix.
+
+None of these re-types the oracle's loop: each compares it with something independent --
+exact rational arithmetic, a closed form, a dense mixing-matrix product, an invariant of
+doubly stochastic matrices, or a special case that collapses to eq. (3)/(6) of PAPER.md.
+Citations are PAPER.md:<line>.  Runs on CPU (-m "not gpu").
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from fixtures import generator as gen
+
+LR, MU = 0.1, 0.9
+
+
+def rand(shape, seed, scale=1.0):
+    rng = np.random.default_rng(seed)
+    return (rng.standard_normal(shape) * scale).astype(np.float32)
+
+
+def bits(a):
+    return np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+
+
+# ------------------------------------------------------------------ pairing / T_k
+
+def paper_T(S, step_k):
+    """T_k built here from the prose, independently of the oracle: even step pairs
+    (2i,2i+1), odd step pairs (2i+1,(2i+2) mod S); averaging a pair puts 0.5 at the four
+    positions (a,a),(a,b),(b,a),(b,b)."""
+    T = np.zeros((S, S))
+    if S == 1:
+        T[0, 0] = 1.0
+        return T
+    for i in range(S // 2):
+        a, b = (2 * i, 2 * i + 1) if step_k % 2 == 0 else (2 * i + 1, (2 * i + 2) % S)
+        for x in (a, b):
+            for y in (a, b):
+                T[x, y] = 0.5
+    return T
+
+
+@pytest.mark.parametrize("S", [2, 4, 6, 8, 16, 64])
+@pytest.mark.parametrize("step_k", [0, 1, 2, 7])
+def test_mixing_matrix_structure(oracle_mod, S, step_k):
+    T = oracle_mod.mixing_matrix(S, step_k)
+    assert np.array_equal(T, T.T)                       # symmetric
+    assert np.array_equal(T.sum(0), np.ones(S))         # doubly stochastic
+    assert np.array_equal(T.sum(1), np.ones(S))
+    assert set(np.unique(T)) <= {0.0, 0.5}
+    assert np.all((T == 0.5).sum(0) == 2) and np.all((T == 0.5).sum(1) == 2)  # "two 0.5s"
+    assert np.array_equal(T @ T, T)                     # pair projector: idempotent
+    assert np.array_equal(T, paper_T(S, step_k))
+    p = oracle_mod.partner(S, step_k)
+    assert np.array_equal(p[p], np.arange(S)) and np.all(p != np.arange(S))  # perfect matching
+    # ring neighbours only: partner is s+1 or s-1 mod S
+    assert np.all(((p - np.arange(S)) % S == 1) | ((p - np.arange(S)) % S == S - 1))
+
+
+def test_pairing_alternates_and_covers_ring(oracle_mod):
+    S = 8
+    even, odd = oracle_mod.partner(S, 0), oracle_mod.partner(S, 1)
+    assert list(even) == [1, 0, 3, 2, 5, 4, 7, 6]
+    assert list(odd) == [7, 2, 1, 4, 3, 6, 5, 0]
+    assert np.array_equal(oracle_mod.partner(S, 10), even)
+    assert np.array_equal(oracle_mod.partner(S, 11), odd)
+    # union of the two matchings is the whole ring (every node talks left and right)
+    edges = {frozenset((s, int(even[s]))) for s in range(S)} | {frozenset((s, int(odd[s]))) for s in range(S)}
+    assert edges == {frozenset((s, (s + 1) % S)) for s in range(S)}
+
+
+def test_pairing_degenerate(oracle_mod):
+    assert list(oracle_mod.partner(1, 0)) == [0]
+    assert list(oracle_mod.partner(2, 0)) == [1, 0]
+    assert list(oracle_mod.partner(2, 1)) == [1, 0]      # S=2: odd pair (1,0) is the same pair
+    for S in (3, 5, 7):
+        with pytest.raises(ValueError):
+            oracle_mod.partner(S, 0)                      # reading R8: no perfect matching
+    with pytest.raises(ValueError):
+        oracle_mod.partner(0, 0)
+
+
+# ------------------------------------------------------------------ eq. (3): plain SGD
+
+def test_reduces_to_eq3_bit_exact(oracle_mod):
+    """S=1, G=1, mu=0: w' = w - lr*g, one fp32 multiply then one fp32 subtract."""
+    P = 4099
+    w, g = rand((1, P), 1, 0.05), rand((1, 1, P), 2, 1e-3)
+    expect_w = w - np.float32(LR) * g[0]          # numpy fp32: mul rounded, then sub rounded
+    v = np.zeros((1, P), np.float32)
+    oracle_mod.step(g, w, v, LR, 0.0, 0)
+    assert np.array_equal(bits(w), bits(expect_w))
+    assert np.array_equal(bits(v), bits(g[0]))     # v = 0*0 + g
+
+
+def test_exact_rational_worked_example(oracle_mod):
+    """Hand-checkable case with dyadic inputs where EVERY fp32 operation is exact, so the
+    expected result is the exact rational value of
+        v' = mu v + (1/G) sum_g g ;  u = w - lr v' ;  w' = (u_s + u_p)/2
+    computed with fractions.Fraction.  Catches a dropped term, a wrong sign, a swapped
+    index or operand (all four super-learners and both learners carry distinct values)."""
+    S, G, P = 4, 2, 3
+    F = Fraction
+    lr, mu = F(1, 2), F(1, 4)
+    w = [[F(s * 8 + i, 16) for i in range(P)] for s in range(S)]
+    v = [[F(-(s + 1) * (i + 2), 32) for i in range(P)] for s in range(S)]
+    g = [[[F((s * 5 + gg * 3 + i * 7) % 11 - 5, 8) for i in range(P)] for gg in range(G)] for s in range(S)]
+    for step_k in (0, 1):
+        wn = np.array([[float(x) for x in r] for r in w], np.float32)
+        vn = np.array([[float(x) for x in r] for r in v], np.float32)
+        gn = np.array([[[float(x) for x in r] for r in q] for q in g], np.float32)
+        oracle_mod.step(gn, wn, vn, float(lr), float(mu), step_k)
+        v = [[mu * v[s][i] + sum(g[s][gg][i] for gg in range(G)) / G for i in range(P)] for s in range(S)]
+        u = [[w[s][i] - lr * v[s][i] for i in range(P)] for s in range(S)]
+        pairs = [(0, 1), (2, 3)] if step_k == 0 else [(1, 2), (3, 0)]
+        w = [[None] * P for _ in range(S)]
+        for a, b in pairs:
+            for i in range(P):
+                w[a][i] = w[b][i] = (u[a][i] + u[b][i]) / 2
+        for s in range(S):
+            for i in range(P):
+                assert F(float(vn[s, i])) == v[s][i], (step_k, s, i)
+                assert F(float(wn[s, i])) == w[s][i], (step_k, s, i)
+
+
+# ------------------------------------------------------------------ momentum closed form (reading R2)
+
+def test_momentum_closed_form(oracle_mod):
+    """Constant gradient g, S=G=1: v_k = g (1-mu^k)/(1-mu),
+    w_k = w_0 - lr g [k - mu (1-mu^k)/(1-mu)]/(1-mu)  (sum of the geometric series)."""
+    P, K = 257, 20
+    w0 = rand((1, P), 3, 0.05)
+    g = rand((1, 1, P), 4, 1e-3)
+    gd, wd = g[0].astype(np.float64), w0.astype(np.float64)
+    lr, mu = np.float64(np.float32(LR)), np.float64(np.float32(MU))   # the fp32 values actually used
+    w32, v32 = w0.copy(), np.zeros((1, P), np.float32)
+    w64, v64 = wd.copy(), np.zeros((1, P), np.float64)
+    for k in range(1, K + 1):
+        oracle_mod.step(g, w32, v32, LR, MU, k - 1)
+        oracle_mod.step_f64(g, w64, v64, float(lr), float(mu), k - 1)
+        v_cf = gd * (1 - mu ** k) / (1 - mu)
+        w_cf = wd - lr * gd * (k - mu * (1 - mu ** k) / (1 - mu)) / (1 - mu)
+        assert np.allclose(v64, v_cf, rtol=1e-12, atol=1e-18)
+        assert np.allclose(w64, w_cf, rtol=1e-12, atol=1e-18)
+        assert np.all(np.abs(w32 - w_cf) <= 1e-6 + 1e-5 * np.abs(w_cf))
+        assert np.all(np.abs(v32 - v_cf) <= 1e-6 + 1e-5 * np.abs(v_cf))
+
+
+# ------------------------------------------------------------------ eq. (4)/(6): the mean
+
+@pytest.mark.parametrize("G", [1, 2, 4])
+def test_mean_of_identical_gradients_is_exact(oracle_mod, G):
+    P = 5003
+    g1 = rand((2, 1, P), 5, 1e-3)
+    gG = np.ascontiguousarray(np.repeat(g1, G, axis=1))
+    w1, v1 = rand((2, P), 6, 0.05), rand((2, P), 7, 0.01)
+    wG, vG = w1.copy(), v1.copy()
+    oracle_mod.step(g1, w1, v1, LR, MU, 0)
+    oracle_mod.step(gG, wG, vG, LR, MU, 0)
+    assert np.array_equal(bits(w1), bits(wG)) and np.array_equal(bits(v1), bits(vG))
+
+
+def test_mean_of_identical_bf16_gradients_exact_for_G8(oracle_mod):
+    """bf16 values have 8 significant bits, so k*g (k<=8) is exact in fp32 and the
+    left-to-right sum of 8 copies times 1/8 returns g exactly."""
+    P, G = 4001, 8
+    gb = gen.f32_to_bf16_bits(rand((2, 1, P), 8, 1e-3))
+    g1f = gen.bf16_bits_to_f32(gb)                       # the same values as fp32 gradients
+    gG = np.ascontiguousarray(np.repeat(gb, G, axis=1))
+    w1, v1 = rand((2, P), 9, 0.05), np.zeros((2, P), np.float32)
+    wG, vG = w1.copy(), v1.copy()
+    oracle_mod.step(g1f, w1, v1, LR, MU, 1)
+    oracle_mod.step(gG, wG, vG, LR, MU, 1)
+    assert np.array_equal(bits(w1), bits(wG)) and np.array_equal(bits(v1), bits(vG))
+
+
+def test_mean_uses_every_learner_once(oracle_mod):
+    """Gradient of learner g is 2^g at element g, 0 elsewhere: the mean must be 2^g/G there
+    (exact), which fails if a learner is dropped, doubled or mis-strided."""
+    S, G = 2, 8
+    g = np.zeros((S, G, G), np.float32)
+    for s in range(S):
+        for k in range(G):
+            g[s, k, k] = 2.0 ** k * (s + 1)
+    w, v = np.zeros((S, G), np.float32), np.zeros((S, G), np.float32)
+    oracle_mod.step(g, w, v, 1.0, 0.0, 0, flags=oracle_mod.NO_MIX)
+    for s in range(S):
+        assert np.array_equal(v[s], (2.0 ** np.arange(G) * (s + 1) / G).astype(np.float32))
+        assert np.array_equal(w[s], -v[s])
+
+
+# ------------------------------------------------------------------ eq. (7): dense T_k brute force
+
+@pytest.mark.parametrize("S,G", [(2, 1), (4, 2), (6, 3), (8, 4)])
+@pytest.mark.parametrize("step_k", [0, 1])
+def test_matches_dense_mixing_matrix(oracle_mod, S, G, step_k):
+    """W' = (W - lr V') T_k with T_k the dense S x S matrix built in THIS file from the
+    prose.  The product is formed in float64 (0.5a+0.5b is exact there) and rounded once,
+    which equals fl32(0.5*fl32(a+b)) barring underflow."""
+    P = 61
+    g, w, v = rand((S, G, P), 10, 1e-3), rand((S, P), 11, 0.05), rand((S, P), 12, 0.01)
+    invG = np.float32(1.0) / np.float32(G)
+    acc = g[:, 0].copy()
+    for k in range(1, G):
+        acc = acc + g[:, k]
+    vn = np.float32(MU) * v + acc * invG
+    u = w - np.float32(LR) * vn                           # columns = learners: U is [S,P] = Theta^T
+    Wd = (paper_T(S, step_k) @ u.astype(np.float64))      # (Theta T)^T = T^T Theta^T = T Theta^T
+    sum32 = np.stack([u[s] + u[int(np.argmax(paper_T(S, step_k)[s] * (np.arange(S) != s)))] for s in range(S)])
+    expect = (np.float32(0.5) * sum32)
+    assert np.allclose(Wd, expect.astype(np.float64), rtol=1e-7, atol=0)   # dense product agrees
+    d = oracle_mod.step(g, w, v, LR, MU, step_k, diag=True)
+    assert np.array_equal(bits(v), bits(vn))
+    assert np.array_equal(bits(w), bits(expect))
+    assert np.max(np.abs(w.astype(np.float64) - Wd)) <= 2 ** -24 * np.max(np.abs(Wd))
+    # diagnostics against numpy in double
+    assert np.allclose(d["gsq"], ((acc * invG).astype(np.float64) ** 2).sum(1), rtol=1e-12)
+    assert np.allclose(d["wsq"], (w.astype(np.float64) ** 2).sum(1), rtol=1e-12)
+    p = oracle_mod.partner(S, step_k)
+    assert np.allclose(d["gap"], ((u.astype(np.float64) - u[p].astype(np.float64)) ** 2).sum(1), rtol=1e-12)
+
+
+def test_eq7_literal_variant_matches_dense(oracle_mod):
+    """Flag EQ7_LITERAL: Theta_{k+1} = Theta_k T_k - lr V' exactly as printed."""
+    S, G, P = 4, 2, 33
+    g, w, v = rand((S, G, P), 13, 1e-3), rand((S, P), 14, 0.05), rand((S, P), 15, 0.01)
+    w64, v64 = w.astype(np.float64), v.astype(np.float64)
+    vn = np.float64(np.float32(MU)) * v64 + g.astype(np.float64).mean(1)
+    expect = paper_T(S, 1) @ w64 - np.float64(np.float32(LR)) * vn
+    oracle_mod.step(g, w, v, LR, MU, 1, flags=oracle_mod.EQ7_LITERAL)
+    assert np.all(np.abs(w - expect) <= 1e-6 + 1e-5 * np.abs(expect))
+    oracle_mod.step_f64(g, w64, v64, float(np.float32(LR)), float(np.float32(MU)), 1,
+                        flags=oracle_mod.EQ7_LITERAL)
+    assert np.allclose(w64, expect, rtol=1e-13, atol=1e-16)
+
+
+# ------------------------------------------------------------------ consensus
+
+@pytest.mark.parametrize("S", [2, 4, 8, 16])
+def test_zero_gradient_preserves_mean_and_contracts(oracle_mod, S):
+    """'If we halt the local updates and only conduct the model averaging ... the system
+    will converge to ... (1/n) sum theta^i'."""
+    P = 501
+    w = rand((S, P), 20 + S, 0.05)
+    w64 = w.astype(np.float64)
+    v, v64 = np.zeros((S, P), np.float32), np.zeros((S, P), np.float64)
+    g = np.zeros((S, 1, P), np.float32)
+    mean0 = w64.mean(0)
+    D_prev = oracle_mod.consensus_distance(w)
+    for k in range(2 * S):
+        oracle_mod.step(g, w, v, LR, MU, k)
+        oracle_mod.step_f64(g, w64, v64, LR, MU, k)
+        assert np.allclose(w64.mean(0), mean0, rtol=0, atol=1e-16)               # exact shadow
+        assert np.max(np.abs(w.astype(np.float64).mean(0) - mean0)) <= (k + 1) * 2 ** -24 * 0.3
+        D = oracle_mod.consensus_distance(w)
+        assert D <= D_prev * (1 + 1e-6)
+        D_prev = D
+        assert not v.any()
+    if S == 2:
+        assert D_prev == 0.0
+    assert D_prev <= 1e-3 * oracle_mod.consensus_distance(rand((S, P), 20 + S, 0.05))
+
+
+def test_consensus_exact_after_one_step_S2_two_steps_S4(oracle_mod):
+    P = 300
+    for S, steps in ((2, 1), (4, 2)):
+        w = rand((S, P), 30 + S, 0.05)
+        v, g = np.zeros((S, P), np.float32), np.zeros((S, 1, P), np.float32)
+        for k in range(steps):
+            oracle_mod.step(g, w, v, LR, MU, k)
+        for s in range(1, S):
+            assert np.array_equal(bits(w[s]), bits(w[0]))     # bitwise consensus
+
+
+@pytest.mark.parametrize("S,rate", [(8, 0.5), (16, 0.8535533905932737)])
+def test_consensus_rate_closed_form(oracle_mod, S, rate):
+    """After step 0 the state is constant on pairs; each (odd, even) double step then acts
+    on the S/2 pair values as the circulant x_i <- (x_{i-1}+2x_i+x_{i+1})/4 with
+    eigenvalues cos^2(pi j/(S/2)).  Seeding the slowest mode j=1 must decay by exactly
+    cos^2(2 pi / S) per double step."""
+    m = S // 2
+    assert abs(np.cos(np.pi / m) ** 2 - rate) < 1e-15
+    P = 4
+    mode = np.cos(2 * np.pi * np.arange(m) / m)
+    w64 = np.repeat(mode, 2)[:, None] * np.ones((1, P))      # constant on even-step pairs
+    v64, g = np.zeros((S, P)), np.zeros((S, 1, P), np.float32)
+    amp0 = np.abs(w64).max()
+    for dbl in range(1, 6):
+        oracle_mod.step_f64(g, w64, v64, LR, MU, 1)            # odd
+        oracle_mod.step_f64(g, w64, v64, LR, MU, 2)            # even
+        assert np.allclose(w64[:, 0], np.repeat(mode, 2) * rate ** dbl, atol=1e-14)
+        assert abs(np.abs(w64).max() / amp0 - rate ** dbl) < 1e-14
+
+
+def test_variance_identity_links_gap_to_consensus(oracle_mod):
+    """D(u) - D(w') = 1/2 sum_pairs ||u_s - u_p||^2  (gap is reported per member, so the
+    sum over s counts each pair twice => 1/4 sum_s gap[s])."""
+    S, G, P = 8, 2, 257
+    g, w, v = rand((S, G, P), 40, 1e-3), rand((S, P), 41, 0.05), rand((S, P), 42, 0.01)
+    wn, vn = w.copy(), v.copy()
+    oracle_mod.step(g, wn, vn, LR, MU, 1, flags=oracle_mod.NO_MIX)    # wn = u
+    D_u = oracle_mod.consensus_distance(wn)
+    d = oracle_mod.step(g, w, v, LR, MU, 1, diag=True)
+    D_w = oracle_mod.consensus_distance(w)
+    assert abs((D_u - D_w) - 0.25 * d["gap"].sum()) <= 1e-6 * D_u
+
+
+# ------------------------------------------------------------------ special cases
+
+def test_ssgd_special_case(oracle_mod):
+    """'ADPSGD has synchronous SGD as its special case': identical weights and
+    identical gradients on every super-learner stay bit-identical to a single learner."""
+    S, G, P, K = 8, 2, 777, 6
+    w1 = rand((1, P), 50, 0.05)
+    v1 = np.zeros((1, P), np.float32)
+    wS, vS = np.repeat(w1, S, 0).copy(), np.repeat(v1, S, 0).copy()
+    for k in range(K):
+        g1 = rand((1, G, P), 60 + k, 1e-3)
+        oracle_mod.step(g1, w1, v1, LR, MU, k)
+        oracle_mod.step(np.ascontiguousarray(np.repeat(g1, S, 0)), wS, vS, LR, MU, k)
+        for s in range(S):
+            assert np.array_equal(bits(wS[s]), bits(w1[0])) and np.array_equal(bits(vS[s]), bits(v1[0]))
+
+
+@pytest.mark.parametrize("G", [2, 3, 4, 8])
+def test_hierarchy_equivalence(oracle_mod, G):
+    """'lambda-learner H-ADPSGD is equivalent to a (lambda/N)-learner ADPSGD':
+    (S,G) equals (S,1) fed the pre-averaged gradient.  Bit-exact when 1/G is a power of
+    two (multiplying by 1.0f afterwards is the identity); G=3 within 1 ulp of gbar."""
+    S, P = 4, 1001
+    g = rand((S, G, P), 70, 1e-3)
+    acc = g[:, 0].copy()
+    for k in range(1, G):
+        acc = acc + g[:, k]
+    gbar = (acc * (np.float32(1.0) / np.float32(G)))[:, None, :].copy()
+    wa, va = rand((S, P), 71, 0.05), rand((S, P), 72, 0.01)
+    wb, vb = wa.copy(), va.copy()
+    oracle_mod.step(g, wa, va, LR, MU, 1)
+    oracle_mod.step(gbar, wb, vb, LR, MU, 1)
+    assert np.array_equal(bits(wa), bits(wb)) and np.array_equal(bits(va), bits(vb))
+
+
+def test_pair_symmetry_and_relabelling(oracle_mod):
+    """Reversing the ring labels maps matchings to matchings; results must be the reversed
+    arrays bit for bit (fp add commutes; no dependence on which member is 's')."""
+    S, G, P = 8, 2, 513
+    g, w, v = rand((S, G, P), 80, 1e-3), rand((S, P), 81, 0.05), rand((S, P), 82, 0.01)
+    # s -> S-1-s maps even pairs (2i,2i+1) onto even pairs, odd pairs onto odd pairs
+    gr, wr, vr = g[::-1].copy(), w[::-1].copy(), v[::-1].copy()
+    for k in (0, 1):
+        oracle_mod.step(g, w, v, LR, MU, k)
+        oracle_mod.step(gr, wr, vr, LR, MU, k)
+        assert np.array_equal(bits(w[::-1]), bits(wr)) and np.array_equal(bits(v[::-1]), bits(vr))
+    po = oracle_mod.partner(S, 1)
+    for s in range(S):
+        assert np.array_equal(bits(w[s]), bits(w[po[s]]))                 # both members get the same bits
+
+
+def test_elementwise_independence_windows(oracle_mod):
+    """The method is element-wise: running on a window equals slicing the full run.  This is
+    what lets full-size GPU parity be checked window by window."""
+    S, G, P = 4, 2, 3000
+    g, w, v = rand((S, G, P), 90, 1e-3), rand((S, P), 91, 0.05), rand((S, P), 92, 0.01)
+    lo, hi = 1234, 2345
+    gw = np.ascontiguousarray(g[:, :, lo:hi])
+    ww, vw = np.ascontiguousarray(w[:, lo:hi]), np.ascontiguousarray(v[:, lo:hi])
+    for k in range(3):
+        oracle_mod.step(g, w, v, LR, MU, k)
+        oracle_mod.step(gw, ww, vw, LR, MU, k)
+    assert np.array_equal(bits(w[:, lo:hi]), bits(ww)) and np.array_equal(bits(v[:, lo:hi]), bits(vw))
+
+
+def test_bf16_gradients_equal_widened_fp32(oracle_mod):
+    S, G, P = 2, 8, 999
+    gb = gen.f32_to_bf16_bits(rand((S, G, P), 95, 1e-3))
+    gf = gen.bf16_bits_to_f32(gb)
+    wa, va = rand((S, P), 96, 0.05), rand((S, P), 97, 0.01)
+    wb, vb = wa.copy(), va.copy()
+    oracle_mod.step(gb, wa, va, LR, MU, 0)
+    oracle_mod.step(gf, wb, vb, LR, MU, 0)
+    assert np.array_equal(bits(wa), bits(wb)) and np.array_equal(bits(va), bits(vb))
+
+
+def test_f32_tracks_f64_shadow_within_north_star_tolerance(oracle_mod):
+    """Tolerance derivation: after 20 steps the fp32 trajectory stays
+    within 1e-6 + 1e-5|w| of the double shadow on config-like data."""
+    S, G, P = 4, 4, 4096
+    w = gen.weights_window(7, S, 0, P)
+    v = np.zeros((S, P), np.float32)
+    w64, v64 = w.astype(np.float64), v.astype(np.float64)
+    for k in range(20):
+        g = gen.grads_window(7, k, S, G, 0, P)
+        oracle_mod.step(g, w, v, LR, MU, k)
+        oracle_mod.step_f64(g, w64, v64, float(np.float32(LR)), float(np.float32(MU)), k)
+    assert np.all(np.abs(w - w64) <= 1e-6 + 1e-5 * np.abs(w64))
+    assert np.all(np.abs(v - v64) <= 1e-6 + 1e-5 * np.abs(v64))
+    assert np.max(np.abs(w - w64)) < 2e-7          # measured head-room, used to justify the bound
+
+
+def test_invalid_arguments(oracle_mod):
+    g, w, v = np.zeros((3, 1, 4), np.float32), np.zeros((3, 4), np.float32), np.zeros((3, 4), np.float32)
+    with pytest.raises(ValueError):
+        oracle_mod.step(g, w, v, LR, MU, 0)               # odd S > 1
+    oracle_mod.step(g, w, v, LR, MU, 0, flags=oracle_mod.NO_MIX)   # fine without mixing
