@@ -1,0 +1,156 @@
+/*
+ * hadpsgd.h -- C ABI of libhadpsgd.so: the per-step super-learner update of
+ * Hierarchical ADPSGD (arxiv 1907.05701), emulated on one B200 (sm_100a).
+ *
+ * One call of hadpsgd_step() performs, for every super-learner s of S, every
+ * parameter i of P, in ONE kernel launch and ONE pass over HBM:
+ *   a2  gbar_s[i] = (1/G) * sum_{g<G} grad_{s,g}[i]        PAPER.md:57 eq. (6), :38 eq. (4), :84 (section 4)
+ *   a3  v_s[i]    = mu * v_s[i] + gbar_s[i]                PAPER.md:34 eq. (3) + momentum (R2)
+ *       u_s[i]    = w_s[i] - lr * v_s[i]
+ *   a4  w_s[i]    = w_p[i] = 1/2 (u_s[i] + u_p[i])         PAPER.md:64-66 eq. (7), T_k; order per :62 (R3)
+ *   a5  diagnostics: sum gbar^2, sum w'^2, sum (u_s-u_p)^2 PAPER.md:72 (consensus)
+ * where p = partner(s, step_k) is the ring neighbour chosen by the pairing
+ * scheduler (a1): even step_k pairs (2i,2i+1), odd pairs (2i+1,(2i+2) mod S).
+ *
+ * Conventions
+ *  - Every function returns an int status: HADPSGD_OK (0) or a negative code.
+ *    No exception crosses this boundary.  Nothing here falls back to the CPU.
+ *  - "dev" pointers are DEVICE pointers, "host" pointers are HOST pointers.
+ *  - The handle owns all descriptor memory.  Device memory is the caller's
+ *    arena when opts->arena != NULL (never freed by the library), else owned
+ *    by the library.  Pointers returned by weights/momentum/grads are
+ *    borrowed and stay valid until hadpsgd_destroy().
+ *  - hadpsgd_step() only enqueues work on the create-time stream and returns.
+ *  - Layout: every buffer (S weight, S momentum, S*G gradient buffers) holds
+ *    P_padded elements; segment k of the caller's table starts at an element
+ *    offset that is a multiple of HADPSGD_SEG_ALIGN_ELEMS in every buffer;
+ *    padding elements are zero at create and stay zero (zero gradient, zero
+ *    weight, zero momentum), so they never perturb results or diagnostics.
+ *    The caller must not write non-zero values into gradient padding.
+ */
+#ifndef HADPSGD_H
+#define HADPSGD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hadpsgd_ctx* hadpsgd_handle; /* opaque */
+
+enum { HADPSGD_F32 = 0, HADPSGD_BF16 = 1 };
+
+enum { /* status codes */
+    HADPSGD_OK = 0,
+    HADPSGD_INVALID_ARG = -1,        /* S<1, S odd and >1 (unless NO_MIX), G<1, n_seg<1, seg_len<1,
+                                        bad dtype, index out of range, NULL out-pointer, S>HADPSGD_MAX_S */
+    HADPSGD_OUT_OF_MEMORY = -2,      /* arena too small / cudaMalloc failed                                */
+    HADPSGD_CUDA = -3,               /* CUDA runtime or launch error; text via hadpsgd_last_error()        */
+    HADPSGD_UNSUPPORTED_DEVICE = -4  /* compute capability != 10.x: no multi-backend dispatch, no fallback */
+};
+
+enum { /* hadpsgd_opts.flags */
+    HADPSGD_DETERMINISTIC = 1u << 0, /* one rounding per fp32 op, no FMA contraction, learners summed
+                                        g=0..G-1: w and v are BIT-EXACT against the oracle               */
+    HADPSGD_NO_MIX        = 1u << 1, /* T_k = I: eq. (6)/(3) only, every super-learner keeps u_s         */
+    HADPSGD_NO_DIAG       = 1u << 2, /* skip a5                                                          */
+    HADPSGD_EQ7_LITERAL   = 1u << 3  /* eq. (7) as printed: w'_s = 1/2 (w_s + w_p) - lr v_s  (row f1)    */
+};
+
+#define HADPSGD_SEG_ALIGN_ELEMS 64 /* 256 B in fp32, 128 B in bf16 */
+#define HADPSGD_MAX_S 512
+
+typedef struct {
+    int32_t grad_dtype;   /* HADPSGD_F32 | HADPSGD_BF16 : dtype of the S*G learner gradient buffers */
+    int32_t master_dtype; /* must be HADPSGD_F32 : weights AND momentum                             */
+} hadpsgd_dtypes;
+
+typedef struct {
+    void*    arena;       /* dev; optional caller-owned memory (e.g. a torch uint8 tensor), 256 B aligned */
+    size_t   arena_bytes; /* >= hadpsgd_required_bytes()                                                   */
+    void*    stream;      /* cudaStream_t; NULL = the legacy default stream                                */
+    uint32_t flags;       /* HADPSGD_DETERMINISTIC | NO_MIX | NO_DIAG | EQ7_LITERAL                        */
+    int32_t  device;      /* CUDA device ordinal; -1 = current device                                      */
+} hadpsgd_opts;
+
+typedef struct { /* host-side copy of the a5 diagnostics of the most recent step */
+    int32_t  S;
+    int32_t  n_pairs;
+    uint64_t step_k;
+    double   gsq[HADPSGD_MAX_S]; /* sum_i gbar_s[i]^2                                  */
+    double   wsq[HADPSGD_MAX_S]; /* sum_i w'_s[i]^2                                    */
+    double   gap[HADPSGD_MAX_S]; /* sum_i (u_s[i]-u_p[i])^2 ; gap[s]==gap[p]; 0 if unpaired */
+} hadpsgd_diag;
+
+/* a0 replica allocator (host only, no GPU needed) ------------------------------------------- */
+
+/* Bytes of device memory hadpsgd_create() needs for this configuration. */
+int hadpsgd_required_bytes(int S, int G, const int64_t* seg_len /*host [n_seg]*/, int n_seg,
+                           hadpsgd_dtypes dt, size_t* out_bytes);
+
+/* The layout the allocator computes: element offset of every segment inside a buffer
+ * (host out [n_seg], may be NULL), padded buffer length in elements, and byte offsets of
+ * the weight, momentum and gradient regions inside the arena (each may be NULL).
+ * weight buffer s   = arena + w_off + s * P_padded * 4
+ * momentum buffer s = arena + v_off + s * P_padded * 4
+ * gradient (s,g)    = arena + g_off + (s*G + g) * P_padded * sizeof(grad_dtype)               */
+int hadpsgd_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
+                   int64_t* seg_offset, int64_t* P_padded,
+                   size_t* w_off, size_t* v_off, size_t* g_off);
+
+/* a1 pairing scheduler (pure host function) -------------------------------------------------- */
+
+/* partner_out[s] = ring neighbour averaged with at step_k.  S==1 -> {0}.  S odd >1 -> INVALID_ARG. */
+int hadpsgd_pairing(int S, uint64_t step_k, int32_t* partner_out /*host [S]*/);
+
+/* lifecycle ---------------------------------------------------------------------------------- */
+
+/* n_seg == 1 is the flat buffer.  opts may be NULL (library-owned memory, default stream,
+ * flags 0, current device).  Weights, momenta, gradients and padding start at zero.          */
+int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
+                   const hadpsgd_opts* opts, hadpsgd_handle* out);
+int hadpsgd_destroy(hadpsgd_handle h);
+
+/* a2-a6 the step ----------------------------------------------------------------------------- */
+
+/* Enqueue one fused step (one kernel launch) on the handle's stream; asynchronous.
+ * Gradient buffers are read-only to the step (not zeroed); w and v are updated in place.
+ * step_k is used only for its parity (no hidden counter: a step can be replayed).           */
+int hadpsgd_step(hadpsgd_handle h, float lr, float momentum, uint64_t step_k);
+
+/* Same step, but with a caller-supplied perfect matching (row f1): partner[s] must satisfy
+ * partner[partner[s]] == s; partner[s] == s leaves s unmixed.                                */
+int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum, uint64_t step_k,
+                          const int32_t* partner /*host [S]*/);
+
+/* End-to-end step from HOST gradients: copies host_grads[s*G+g] (host, P_padded elements of
+ * grad_dtype each, ideally pinned) to the device chunk by chunk, overlapping the copies with
+ * the fused kernel on element sub-ranges, then copies the diagnostics back into *diag_out
+ * (may be NULL) and synchronises the stream.                                                */
+int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads /*host [S*G]*/,
+                      float lr, float momentum, uint64_t step_k, hadpsgd_diag* diag_out);
+
+/* accessors (borrowed device pointers; no copy, no sync) ------------------------------------- */
+int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr);
+int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr);
+int hadpsgd_grads(hadpsgd_handle h, int s, int g, void** dev_ptr);
+int hadpsgd_segment(hadpsgd_handle h, int seg, int64_t* elem_offset, int64_t* elem_len);
+int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded);
+
+/* Synchronises the stream and copies the diagnostics of the most recent step to the host. */
+int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out);
+
+/* Tuning knobs for measurement (persistent grid size, block size, tile order); 0 = default. */
+int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm, int threads_per_block, int variant);
+/* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
+int hadpsgd_launch_count(hadpsgd_handle h, uint64_t* out);
+
+const char* hadpsgd_error_string(int code);
+const char* hadpsgd_last_error(hadpsgd_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

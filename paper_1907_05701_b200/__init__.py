@@ -1,0 +1,7 @@
+"""paper_1907_05701_b200 -- B200-native super-learner step of Hierarchical ADPSGD.
+
+The product is libhadpsgd.so (hand-written sm_100a CUDA behind the C ABI of
+include/hadpsgd.h); this package is its thin Python binding.  No CPU fallback.
+"""
+from .binding import (BF16, DETERMINISTIC, EQ7_LITERAL, F32, NO_DIAG, NO_MIX, Hadpsgd, HadpsgdError,  # noqa: F401
+                      hadpsgd_layout, hadpsgd_pairing, hadpsgd_required_bytes, lib)

@@ -1,0 +1,342 @@
+// hadpsgd.cu -- B2/B1: the C ABI of include/hadpsgd.h over the fused step kernel.
+// sm_100a only: hadpsgd_create() refuses any device whose compute capability is not 10.x.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "internal.h"
+#include "step_kernel.cuh"
+
+using namespace hadpsgd;
+
+struct hadpsgd_ctx {
+    Layout L;
+    uint32_t flags = 0;
+    int device = 0;
+    int num_sms = 0;
+    cudaStream_t stream = nullptr;
+    cudaStream_t copy_stream = nullptr;   // host path: H2D copies overlap the kernel
+    std::vector<cudaEvent_t> chunk_events;
+    char* arena = nullptr;
+    bool owns_arena = false;
+    double* d_partials = nullptr;
+    double* d_diag = nullptr;
+    unsigned int* d_ticket = nullptr;
+    uint64_t last_step_k = 0;
+    int last_n_pairs = 0;
+    uint64_t launches = 0;
+    int blocks_per_sm = 0, threads = 0, variant = 0;   // tuning overrides (0 = default)
+    std::string err;
+};
+
+static thread_local std::string g_create_error;
+
+#define CUDA_TRY(h, call)                                                                   \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            (h)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                  \
+            return HADPSGD_CUDA;                                                            \
+        }                                                                                   \
+    } while (0)
+
+// ---- kernel dispatch -------------------------------------------------------------------
+namespace {
+
+struct LaunchPlan { const void* fn; int threads; };
+
+template <int G, bool BF16, bool EXACT, bool DIAG, int MODE>
+LaunchPlan plan_for() {
+    // Register budget: 2G+4 (fp32) / 2G+8 (bf16) 16-byte loads are live at once.
+    constexpr int loads = (MODE == kSingle ? 1 : 2) * ((G > 0 ? G : 4) + (BF16 ? 4 : 2));
+    constexpr int THREADS = 256;
+    constexpr int MINB = loads <= 6 ? 4 : (loads <= 12 ? 3 : (loads <= 20 ? 2 : 1));
+    return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, THREADS, MINB>), THREADS};
+}
+
+template <int G, bool BF16, bool EXACT, bool DIAG>
+LaunchPlan pick_mode(int mode) {
+    switch (mode) {
+        case kPair: return plan_for<G, BF16, EXACT, DIAG, kPair>();
+        case kSingle: return plan_for<G, BF16, EXACT, DIAG, kSingle>();
+        default: return plan_for<G, BF16, EXACT, DIAG, kPairEq7>();
+    }
+}
+template <int G, bool BF16>
+LaunchPlan pick_flags(bool exact, bool diag, int mode) {
+    if (exact) return diag ? pick_mode<G, BF16, true, true>(mode) : pick_mode<G, BF16, true, false>(mode);
+    return diag ? pick_mode<G, BF16, false, true>(mode) : pick_mode<G, BF16, false, false>(mode);
+}
+template <bool BF16>
+LaunchPlan pick_G(int G, bool exact, bool diag, int mode) {
+    switch (G) {
+        case 1: return pick_flags<1, BF16>(exact, diag, mode);
+        case 2: return pick_flags<2, BF16>(exact, diag, mode);
+        case 4: return pick_flags<4, BF16>(exact, diag, mode);
+        case 8: return pick_flags<8, BF16>(exact, diag, mode);
+        default: return pick_flags<0, BF16>(exact, diag, mode);  // runtime learner count
+    }
+}
+
+int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, float lr, float mu,
+                 int64_t elem_begin, int64_t elem_end, bool accumulate) {
+    if (items.empty() || elem_end <= elem_begin) return HADPSGD_OK;
+    const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
+    const bool exact = h->flags & HADPSGD_DETERMINISTIC;
+    const bool diag = !(h->flags & HADPSGD_NO_DIAG);
+    LaunchPlan plan = bf16 ? pick_G<true>(h->L.G, exact, diag, mode) : pick_G<false>(h->L.G, exact, diag, mode);
+
+    const int unit = bf16 ? 8 : 4;
+    StepArgs a;
+    a.w = reinterpret_cast<float*>(h->arena + h->L.w_off);
+    a.v = reinterpret_cast<float*>(h->arena + h->L.v_off);
+    a.g = h->arena + h->L.g_off;
+    a.P = h->L.P_padded;
+    a.unit_begin = elem_begin / unit;
+    a.unit_end = elem_end / unit;
+    a.G = h->L.G;
+    a.n_work = static_cast<int>(items.size());
+    a.lr = lr; a.mu = mu;
+    a.invG = 1.0f / static_cast<float>(h->L.G);   // fp32 reciprocal, exact for G = 1,2,4,8 (R5)
+    a.accumulate_diag = accumulate ? 1 : 0;
+    a.S = h->L.S;
+    a.partials = h->d_partials; a.diag = h->d_diag; a.ticket = h->d_ticket;
+    for (size_t j = 0; j < items.size(); ++j) a.work[j] = make_short2(static_cast<short>(items[j].a), static_cast<short>(items[j].b));
+
+    int occ = 0;
+    CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, 0));
+    if (occ < 1) occ = 1;
+    if (h->blocks_per_sm > 0) occ = h->blocks_per_sm;
+    long long n_units = a.unit_end - a.unit_begin;
+    long long want = (n_units + plan.threads - 1) / plan.threads;
+    long long grid = static_cast<long long>(h->num_sms) * occ;
+    if (grid > want) grid = want;
+    if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;
+    if (grid < 1) grid = 1;
+
+    void* params[] = {&a};
+    CUDA_TRY(h, cudaLaunchKernel(plan.fn, dim3(static_cast<unsigned>(grid)), dim3(plan.threads), params, 0, h->stream));
+    h->launches++;
+    return HADPSGD_OK;
+}
+
+// One step over [elem_begin, elem_end) for an arbitrary matching.
+int step_range(hadpsgd_ctx* h, const int32_t* partner, float lr, float mu, int64_t elem_begin,
+               int64_t elem_end, bool accumulate) {
+    std::vector<WorkItem> pairs, singles;
+    matching_to_work(h->L.S, partner, &pairs, &singles);
+    h->last_n_pairs = static_cast<int>(pairs.size());
+    const int pair_mode = (h->flags & HADPSGD_EQ7_LITERAL) ? kPairEq7 : kPair;
+    int rc = launch_items(h, pairs, pair_mode, lr, mu, elem_begin, elem_end, accumulate);
+    if (rc != HADPSGD_OK) return rc;
+    // unmixed super-learners (S == 1, NO_MIX, or partner[s] == s in a custom matching)
+    return launch_items(h, singles, kSingle, lr, mu, elem_begin, elem_end, accumulate);
+}
+
+int build_partner(hadpsgd_ctx* h, uint64_t step_k, const int32_t* custom, std::vector<int32_t>* partner) {
+    const int S = h->L.S;
+    partner->resize(S);
+    if (custom) {
+        if (validate_matching(S, custom) != HADPSGD_OK) { h->err = "partner[] is not a matching"; return HADPSGD_INVALID_ARG; }
+        std::memcpy(partner->data(), custom, sizeof(int32_t) * S);
+    } else if (h->flags & HADPSGD_NO_MIX) {
+        for (int s = 0; s < S; ++s) (*partner)[s] = s;
+    } else if (ring_partner(S, step_k, partner->data()) != HADPSGD_OK) {
+        h->err = "no perfect ring matching for odd S > 1";
+        return HADPSGD_INVALID_ARG;
+    }
+    return HADPSGD_OK;
+}
+
+}  // namespace
+
+// ---- C ABI -----------------------------------------------------------------------------
+
+extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
+                              const hadpsgd_opts* opts, hadpsgd_handle* out) {
+    if (!out) { g_create_error = "out handle is NULL"; return HADPSGD_INVALID_ARG; }
+    *out = nullptr;
+    Layout L;
+    std::string why;
+    int rc = compute_layout(S, G, seg_len, n_seg, dt, &L, &why);
+    if (rc != HADPSGD_OK) { g_create_error = why; return rc; }
+    const uint32_t flags = opts ? opts->flags : 0u;
+    if (S > 1 && (S & 1) && !(flags & HADPSGD_NO_MIX)) {
+        g_create_error = "odd S > 1 has no perfect ring matching (PAPER.md:66 needs two 0.5s per row; use HADPSGD_NO_MIX for unmixed runs)";
+        return HADPSGD_INVALID_ARG;
+    }
+
+    int dev = (opts && opts->device >= 0) ? opts->device : -1;
+    cudaError_t e;
+    if (dev < 0) { e = cudaGetDevice(&dev); } else { e = cudaSetDevice(dev); }
+    if (e != cudaSuccess) { g_create_error = std::string("no CUDA device: ") + cudaGetErrorString(e); return HADPSGD_CUDA; }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) { g_create_error = cudaGetErrorString(e); return HADPSGD_CUDA; }
+    if (prop.major != 10) {
+        g_create_error = "libhadpsgd is built for sm_100a only; device is sm_" + std::to_string(prop.major) + std::to_string(prop.minor);
+        return HADPSGD_UNSUPPORTED_DEVICE;
+    }
+
+    hadpsgd_ctx* h = new hadpsgd_ctx();
+    h->L = L; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount;
+    h->stream = opts ? static_cast<cudaStream_t>(opts->stream) : nullptr;
+    if (opts && opts->arena) {
+        if (opts->arena_bytes < L.total_bytes || (reinterpret_cast<uintptr_t>(opts->arena) % kRegionAlign) != 0) {
+            g_create_error = "arena too small or not 256 B aligned"; delete h; return HADPSGD_OUT_OF_MEMORY;
+        }
+        h->arena = static_cast<char*>(opts->arena);
+    } else {
+        void* p = nullptr;
+        e = cudaMalloc(&p, L.total_bytes);
+        if (e != cudaSuccess) { g_create_error = std::string("cudaMalloc: ") + cudaGetErrorString(e); delete h; return HADPSGD_OUT_OF_MEMORY; }
+        h->arena = static_cast<char*>(p); h->owns_arena = true;
+    }
+    e = cudaMemsetAsync(h->arena, 0, L.total_bytes, h->stream);   // zero w, v, grads, padding, scratch
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) {
+        g_create_error = std::string("init: ") + cudaGetErrorString(e);
+        if (h->owns_arena) cudaFree(h->arena);
+        delete h; return HADPSGD_CUDA;
+    }
+    char* aux = h->arena + L.aux_off;
+    h->d_partials = reinterpret_cast<double*>(aux);
+    h->d_diag = h->d_partials + static_cast<size_t>(S) * kDiagQuantities * kMaxGridBlocks;
+    h->d_ticket = reinterpret_cast<unsigned int*>(h->d_diag + 3 * S);
+    *out = h;
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_destroy(hadpsgd_handle h) {
+    if (!h) return HADPSGD_INVALID_ARG;
+    cudaStreamSynchronize(h->stream);
+    for (cudaEvent_t ev : h->chunk_events) cudaEventDestroy(ev);
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    if (h->owns_arena) cudaFree(h->arena);
+    delete h;
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_step(hadpsgd_handle h, float lr, float momentum, uint64_t step_k) {
+    return hadpsgd_step_matching(h, lr, momentum, step_k, nullptr);
+}
+
+extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum, uint64_t step_k,
+                                     const int32_t* partner) {
+    if (!h) return HADPSGD_INVALID_ARG;
+    std::vector<int32_t> pt;
+    int rc = build_partner(h, step_k, partner, &pt);
+    if (rc != HADPSGD_OK) return rc;
+    h->last_step_k = step_k;
+    return step_range(h, pt.data(), lr, momentum, 0, h->L.P_padded, false);
+}
+
+extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads, float lr,
+                                 float momentum, uint64_t step_k, hadpsgd_diag* diag_out) {
+    if (!h || !host_grads) return HADPSGD_INVALID_ARG;
+    std::vector<int32_t> pt;
+    int rc = build_partner(h, step_k, nullptr, &pt);
+    if (rc != HADPSGD_OK) return rc;
+    h->last_step_k = step_k;
+    const int n_buf = h->L.S * h->L.G;
+    for (int b = 0; b < n_buf; ++b) if (!host_grads[b]) { h->err = "host_grads[] has a NULL entry"; return HADPSGD_INVALID_ARG; }
+
+    // Chunk the element range so the H2D copy of chunk c+1 overlaps the kernel on chunk c.
+    const int64_t P = h->L.P_padded;
+    const size_t eb = h->L.grad_elem_bytes();
+    int64_t chunk = (int64_t(8) << 20);                       // 8 Mi elements per learner per chunk
+    chunk = chunk / HADPSGD_SEG_ALIGN_ELEMS * HADPSGD_SEG_ALIGN_ELEMS;
+    const int n_chunks = static_cast<int>((P + chunk - 1) / chunk);
+    while (static_cast<int>(h->chunk_events.size()) < n_chunks + 1) {
+        cudaEvent_t ev;
+        CUDA_TRY(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        h->chunk_events.push_back(ev);
+    }
+    // the copy stream must not overwrite gradients an earlier step on h->stream still reads
+    CUDA_TRY(h, cudaEventRecord(h->chunk_events[n_chunks], h->stream));
+    CUDA_TRY(h, cudaStreamWaitEvent(h->copy_stream, h->chunk_events[n_chunks], 0));
+    char* gdev = h->arena + h->L.g_off;
+    for (int c = 0; c < n_chunks; ++c) {
+        const int64_t e0 = c * chunk, e1 = (e0 + chunk < P) ? e0 + chunk : P;
+        for (int b = 0; b < n_buf; ++b)
+            CUDA_TRY(h, cudaMemcpyAsync(gdev + static_cast<size_t>(b) * h->L.g_stride_bytes() + e0 * eb,
+                                        static_cast<const char*>(host_grads[b]) + e0 * eb,
+                                        static_cast<size_t>(e1 - e0) * eb, cudaMemcpyHostToDevice, h->copy_stream));
+        CUDA_TRY(h, cudaEventRecord(h->chunk_events[c], h->copy_stream));
+        CUDA_TRY(h, cudaStreamWaitEvent(h->stream, h->chunk_events[c], 0));
+        rc = step_range(h, pt.data(), lr, momentum, e0, e1, c > 0);
+        if (rc != HADPSGD_OK) return rc;
+    }
+    if (diag_out) return hadpsgd_diagnostics(h, diag_out);
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr) {
+    if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
+    *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.w_off + static_cast<size_t>(s) * h->L.w_stride_bytes());
+    return HADPSGD_OK;
+}
+extern "C" int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr) {
+    if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
+    *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.v_off + static_cast<size_t>(s) * h->L.w_stride_bytes());
+    return HADPSGD_OK;
+}
+extern "C" int hadpsgd_grads(hadpsgd_handle h, int s, int g, void** dev_ptr) {
+    if (!h || !dev_ptr || s < 0 || s >= h->L.S || g < 0 || g >= h->L.G) return HADPSGD_INVALID_ARG;
+    *dev_ptr = h->arena + h->L.g_off + (static_cast<size_t>(s) * h->L.G + g) * h->L.g_stride_bytes();
+    return HADPSGD_OK;
+}
+extern "C" int hadpsgd_segment(hadpsgd_handle h, int seg, int64_t* elem_offset, int64_t* elem_len) {
+    if (!h || seg < 0 || seg >= h->L.n_seg) return HADPSGD_INVALID_ARG;
+    if (elem_offset) *elem_offset = h->L.seg_offset[seg];
+    if (elem_len) *elem_len = h->L.seg_len[seg];
+    return HADPSGD_OK;
+}
+extern "C" int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded) {
+    if (!h || !P_padded) return HADPSGD_INVALID_ARG;
+    *P_padded = h->L.P_padded;
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
+    if (!h || !host_out) return HADPSGD_INVALID_ARG;
+    if (h->flags & HADPSGD_NO_DIAG) { h->err = "handle was created with HADPSGD_NO_DIAG"; return HADPSGD_INVALID_ARG; }
+    const int S = h->L.S;
+    std::vector<double> tmp(3 * S);
+    CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * 3 * S, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    host_out->S = S; host_out->n_pairs = h->last_n_pairs; host_out->step_k = h->last_step_k;
+    std::memcpy(host_out->gsq, tmp.data(), sizeof(double) * S);
+    std::memcpy(host_out->wsq, tmp.data() + S, sizeof(double) * S);
+    std::memcpy(host_out->gap, tmp.data() + 2 * S, sizeof(double) * S);
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm, int threads_per_block, int variant) {
+    if (!h || blocks_per_sm < 0 || blocks_per_sm > 16) return HADPSGD_INVALID_ARG;
+    h->blocks_per_sm = blocks_per_sm; h->threads = threads_per_block; h->variant = variant;
+    return HADPSGD_OK;
+}
+extern "C" int hadpsgd_launch_count(hadpsgd_handle h, uint64_t* out) {
+    if (!h || !out) return HADPSGD_INVALID_ARG;
+    *out = h->launches;
+    return HADPSGD_OK;
+}
+
+extern "C" const char* hadpsgd_error_string(int code) {
+    switch (code) {
+        case HADPSGD_OK: return "ok";
+        case HADPSGD_INVALID_ARG: return "invalid argument";
+        case HADPSGD_OUT_OF_MEMORY: return "out of device memory";
+        case HADPSGD_CUDA: return "CUDA error";
+        case HADPSGD_UNSUPPORTED_DEVICE: return "unsupported device (sm_100a required)";
+        default: return "unknown status";
+    }
+}
+extern "C" const char* hadpsgd_last_error(hadpsgd_handle h) {
+    return h ? h->err.c_str() : g_create_error.c_str();
+}

@@ -1,0 +1,381 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  All tests here need a B200 (-m gpu).
+
+Bars (north_star):  DETERMINISTIC mode -> w and v bit-exact.  Default mode ->
+|d| <= 1e-6 + 1e-5 |x| per element.  Diagnostics -> relative 1e-4 (reduction order is free).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+LR, MU = 0.1, 0.9
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def H(torch_cuda):
+    import paper_1907_05701_b200 as m
+    m.lib()                      # fail loudly if the extension is missing
+    return m
+
+
+def bits(a):
+    return np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+
+
+def run_both(H, oracle_mod, S, G, seg_len, steps, *, bf16=False, flags=0, seed=11, dist="normal",
+             matching=None, lr=LR, mu=MU, check_diag=True, v0_sd=0.0, blocks_per_sm=0):
+    """Run `steps` steps on the GPU and in the oracle over the WHOLE (small) problem and return
+    (gpu_w, gpu_v, ora_w, ora_v) in natural order; asserts diagnostics on the way."""
+    import torch
+    from fixtures import generator as gen
+    from fixtures import problem
+    exact = bool(flags & H.DETERMINISTIC)
+    h = H.Hadpsgd(S, G, seg_len, H.BF16 if bf16 else H.F32, flags)
+    if blocks_per_sm:
+        h.hadpsgd_set_launch(blocks_per_sm)
+    P = int(sum(seg_len))
+    problem.fill_weights(h, seed)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    nat = torch.from_numpy(h.natural_index()).cuda()
+    if v0_sd:
+        for s in range(S):
+            v0 = gen.normal_f32(gen.stream_key(seed, gen.STREAM_MOMENTUM, 0, s, 0), 0, P, v0_sd)
+            ov[s] = v0
+            h.hadpsgd_momentum(s)[nat] = torch.from_numpy(v0).cuda()
+    oflags = 0
+    if flags & H.NO_MIX: oflags |= oracle_mod.NO_MIX
+    if flags & H.EQ7_LITERAL: oflags |= oracle_mod.EQ7_LITERAL
+    for k in range(steps):
+        problem.fill_grads(h, seed, k, dist)
+        og = problem.host_grads(seed, k, S, G, 0, P, dist, bf16=bf16)
+        if matching is not None:
+            h.hadpsgd_step_matching(lr, mu, k, matching(k))
+        else:
+            h.hadpsgd_step(lr, mu, k)
+        od = oracle_mod.step(og, ow, ov, lr, mu, k, flags=oflags, diag=True)
+        if check_diag and not (flags & H.NO_DIAG) and matching is None:
+            gd = h.hadpsgd_diagnostics()
+            for name in ("gsq", "wsq", "gap"):
+                assert np.allclose(gd[name], od[name], rtol=1e-4, atol=1e-30), (name, k, gd[name], od[name])
+    torch.cuda.synchronize()
+    gw = np.stack([h.hadpsgd_weights(s)[nat].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[nat].cpu().numpy() for s in range(S)])
+    # padding must still be zero
+    if h.P_padded != P:
+        mask = torch.ones(h.P_padded, dtype=torch.bool, device="cuda"); mask[nat] = False
+        for s in range(S):
+            assert not h.hadpsgd_weights(s)[mask].any() and not h.hadpsgd_momentum(s)[mask].any()
+    h.close()
+    return gw, gv, ow, ov
+
+
+def assert_parity(gw, gv, ow, ov, exact):
+    if exact:
+        assert np.array_equal(bits(gw), bits(ow)), f"w differs in {np.sum(bits(gw) != bits(ow))} elements"
+        assert np.array_equal(bits(gv), bits(ov)), f"v differs in {np.sum(bits(gv) != bits(ov))} elements"
+    else:
+        assert np.all(np.abs(gw - ow) <= 1e-6 + 1e-5 * np.abs(ow)), np.max(np.abs(gw - ow))
+        assert np.all(np.abs(gv - ov) <= 1e-6 + 1e-5 * np.abs(ov)), np.max(np.abs(gv - ov))
+
+
+# ------------------------------------------------------------------------------- fixtures
+
+def test_device_generator_matches_host(torch_cuda):
+    torch = torch_cuda
+    from fixtures import device, generator as gen
+    key = gen.stream_key(5, gen.STREAM_GRAD, 3, 2, 1)
+    n, off = 100_003, 1_234_567_891
+    for dist, scale in (("normal", 1e-3), ("uniform", 1e-3), ("normal", 0.05)):
+        t = torch.empty(n, dtype=torch.float32, device="cuda")
+        device.fill(t, key, dist, scale, elem_offset=off)
+        ref = gen.normal_f32(key, off, n, scale) if dist == "normal" else gen.uniform_f32(key, off, n, scale)
+        assert np.array_equal(bits(t.cpu().numpy()), bits(ref))
+    tb = torch.empty(n, dtype=torch.bfloat16, device="cuda")
+    device.fill(tb, key, "normal", 1e-3, elem_offset=off)
+    assert np.array_equal(tb.view(torch.int16).cpu().numpy().view(np.uint16), gen.normal_bf16(key, off, n, 1e-3))
+
+
+# ------------------------------------------------------------------------------- config 0: Tiny
+
+@pytest.mark.parametrize("exact", [True, False])
+def test_tiny_config_full(H, oracle_mod, exact):
+    """BASELINE.json configs[0]: S=2, G=2, flat 1,000,000 fp32, lr 0.1, mu 0.9, 10 steps."""
+    flags = H.DETERMINISTIC if exact else 0
+    gw, gv, ow, ov = run_both(H, oracle_mod, 2, 2, [1_000_000], 10, flags=flags, seed=1)
+    assert_parity(gw, gv, ow, ov, exact)
+
+
+# ------------------------------------------------------------------------------- shapes / edge cases
+
+ODD_TABLE = [1, 3, 7, 1025, 64, 63, 65, 4099, 2, 100_001]      # adversarial ragged table
+
+
+@pytest.mark.parametrize("S,G", [(1, 1), (2, 1), (2, 2), (4, 3), (4, 4), (6, 5), (8, 8), (16, 4), (2, 16), (2, 13)])
+@pytest.mark.parametrize("bf16", [False, True])
+def test_small_shapes_bit_exact(H, oracle_mod, S, G, bf16):
+    """Templated G in {1,2,4,8} and the runtime-G kernel (3,5,13,16); several tiles plus a
+    ragged tail (P = 70,001 is not a multiple of anything); deterministic => bit-exact."""
+    gw, gv, ow, ov = run_both(H, oracle_mod, S, G, [70_001], 3, bf16=bf16, flags=H.DETERMINISTIC, seed=S * 100 + G,
+                              v0_sd=0.01)
+    assert_parity(gw, gv, ow, ov, True)
+
+
+@pytest.mark.parametrize("bf16", [False, True])
+@pytest.mark.parametrize("exact", [True, False])
+def test_ragged_table_equals_flat(H, oracle_mod, bf16, exact):
+    """Odd-length segment table: padded layout, padding stays zero, results equal the oracle on
+    the concatenated (flat) data."""
+    flags = H.DETERMINISTIC if exact else 0
+    gw, gv, ow, ov = run_both(H, oracle_mod, 4, 2, ODD_TABLE, 4, bf16=bf16, flags=flags, seed=21)
+    assert_parity(gw, gv, ow, ov, exact)
+    if exact:   # and the flat layout gives the very same bits
+        fw, fv, _, _ = run_both(H, oracle_mod, 4, 2, [sum(ODD_TABLE)], 4, bf16=bf16, flags=flags, seed=21)
+        assert np.array_equal(bits(fw), bits(gw)) and np.array_equal(bits(fv), bits(gv))
+
+
+@pytest.mark.parametrize("P", [1, 3, 4, 5, 63, 64, 65, 1023, 1024, 1025])
+def test_tiny_lengths(H, oracle_mod, P):
+    gw, gv, ow, ov = run_both(H, oracle_mod, 2, 2, [P], 2, flags=H.DETERMINISTIC, seed=P)
+    assert_parity(gw, gv, ow, ov, True)
+
+
+@pytest.mark.parametrize("flagname", ["NO_MIX", "EQ7_LITERAL", "NO_DIAG"])
+@pytest.mark.parametrize("bf16", [False, True])
+def test_flags(H, oracle_mod, flagname, bf16):
+    flags = H.DETERMINISTIC | getattr(H, flagname)
+    gw, gv, ow, ov = run_both(H, oracle_mod, 4, 4, [33_333], 3, bf16=bf16, flags=flags, seed=31, v0_sd=0.01)
+    assert_parity(gw, gv, ow, ov, True)
+    gw, gv, ow, ov = run_both(H, oracle_mod, 4, 4, [33_333], 3, bf16=bf16, flags=getattr(H, flagname), seed=31)
+    assert_parity(gw, gv, ow, ov, False)
+
+
+def test_odd_S_without_mixing(H, oracle_mod):
+    gw, gv, ow, ov = run_both(H, oracle_mod, 3, 2, [10_000], 2, flags=H.DETERMINISTIC | H.NO_MIX, seed=41)
+    assert_parity(gw, gv, ow, ov, True)
+
+
+def test_max_S(H, oracle_mod):
+    """S = HADPSGD_MAX_S = 512 super-learners (256 pairs in the kernel's work table)."""
+    gw, gv, ow, ov = run_both(H, oracle_mod, 512, 1, [2_000], 2, flags=H.DETERMINISTIC, seed=51)
+    assert_parity(gw, gv, ow, ov, True)
+
+
+def test_default_mode_tolerance_20_steps(H, oracle_mod):
+    gw, gv, ow, ov = run_both(H, oracle_mod, 16, 4, [50_000], 20, seed=61)
+    assert_parity(gw, gv, ow, ov, False)
+
+
+def test_forced_grid_sizes(H, oracle_mod):
+    """Same bits whatever the persistent grid (1 block/SM ... 8 blocks/SM)."""
+    ref = None
+    for bps in (1, 2, 8):
+        gw, gv, ow, ov = run_both(H, oracle_mod, 4, 4, [300_007], 2, flags=H.DETERMINISTIC, seed=71, blocks_per_sm=bps)
+        assert_parity(gw, gv, ow, ov, True)
+
+
+def test_uniform_sweep_points(H, oracle_mod):
+    """BASELINE.json configs[4] (bandwidth sweep) sample points small enough for a full
+    oracle run: flat fp32, uniform grads in [-1e-3, 1e-3]."""
+    for P, S, G in ((1 << 10, 2, 2), (1 << 12, 16, 8), (1 << 14, 4, 4), (1 << 16, 8, 2), (1 << 18, 2, 8)):
+        gw, gv, ow, ov = run_both(H, oracle_mod, S, G, [P], 3, flags=H.DETERMINISTIC, seed=P + S + G, dist="uniform")
+        assert_parity(gw, gv, ow, ov, True)
+
+
+# ------------------------------------------------------------------------------- API behaviour
+
+def test_custom_matching_and_unpaired(H, oracle_mod):
+    """hadpsgd_step_matching (row f1): caller-supplied matching, including unpaired members.
+    Oracle side: the step is element-wise and pair-local, so it is assembled from oracle runs
+    on the sub-rings {pair} (S=2) and {single} (S=1)."""
+    import torch
+    from fixtures import problem
+    S, G, P, seed = 6, 2, 20_000, 81
+    partner = [3, 1, 5, 0, 4, 2]                      # pairs (0,3), (2,5); 1 and 4 unmixed
+    h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
+    problem.fill_weights(h, seed)
+    problem.fill_grads(h, seed, 0)
+    h.hadpsgd_step_matching(LR, MU, 0, partner)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    og = problem.host_grads(seed, 0, S, G, 0, P)
+    for grp in ([0, 3], [2, 5], [1], [4]):
+        w, v, g = ow[grp].copy(), ov[grp].copy(), np.ascontiguousarray(og[grp])
+        oracle_mod.step(g, w, v, LR, MU, 0)
+        ow[grp], ov[grp] = w, v
+    torch.cuda.synchronize()
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    assert_parity(gw, gv, ow, ov, True)
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_step_matching(LR, MU, 0, [1, 2, 0, 3, 4, 5])     # not an involution
+    h.close()
+
+
+def test_host_gradient_path_equals_resident_path(H, oracle_mod):
+    """hadpsgd_step_host (the e2e entry): chunked H2D + kernel on element sub-ranges must give
+    the same bits and the same diagnostics as the resident-gradient step.  P spans 3 chunks."""
+    import torch
+    from fixtures import problem
+    S, G, seed = 2, 2, 91
+    P = (8 << 20) * 2 + 12_345 * 64
+    outs = []
+    for path in ("resident", "host"):
+        h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
+        problem.fill_weights(h, seed)
+        for k in range(2):
+            problem.fill_grads(h, seed, k)
+            if path == "resident":
+                h.hadpsgd_step(LR, MU, k)
+                d = h.hadpsgd_diagnostics()
+            else:
+                host = [h.hadpsgd_grads(s, g).cpu().pin_memory() for s in range(S) for g in range(G)]
+                for s in range(S):
+                    for g in range(G):
+                        h.hadpsgd_grads(s, g).zero_()          # the copy must really happen
+                d = h.hadpsgd_step_host([t.data_ptr() for t in host], LR, MU, k)
+        torch.cuda.synchronize()
+        outs.append((torch.stack([h.hadpsgd_weights(s) for s in range(S)]).cpu().numpy(),
+                     torch.stack([h.hadpsgd_momentum(s) for s in range(S)]).cpu().numpy(), d))
+        h.close()
+    assert np.array_equal(bits(outs[0][0]), bits(outs[1][0])) and np.array_equal(bits(outs[0][1]), bits(outs[1][1]))
+    for name in ("gsq", "wsq", "gap"):
+        assert np.allclose(outs[0][2][name], outs[1][2][name], rtol=1e-12)
+    # sampled window against the oracle
+    lo, hi = P - 5000, P
+    ow, ov = problem.host_weights(seed, S, lo, hi), np.zeros((S, hi - lo), np.float32)
+    for k in range(2):
+        oracle_mod.step(problem.host_grads(seed, k, S, G, lo, hi), ow, ov, LR, MU, k)
+    assert np.array_equal(bits(outs[1][0][:, lo:hi]), bits(ow))
+
+
+def test_diagnostics_are_run_to_run_deterministic(H):
+    from fixtures import problem
+    res = []
+    for _ in range(3):
+        h = H.Hadpsgd(4, 4, [1_000_003], H.F32, 0)
+        problem.fill_weights(h, 5)
+        problem.fill_grads(h, 5, 0)
+        h.hadpsgd_step(LR, MU, 1)
+        d = h.hadpsgd_diagnostics()
+        res.append(np.concatenate([d["gsq"], d["wsq"], d["gap"]]))
+        h.close()
+    assert np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
+
+
+def test_error_codes(H, torch_cuda):
+    torch = torch_cuda
+    with pytest.raises(H.HadpsgdError) as e:
+        H.Hadpsgd(3, 2, [100])                                   # odd S > 1
+    assert e.value.code == -1
+    with pytest.raises(H.HadpsgdError):
+        H.Hadpsgd(2, 0, [100])
+    with pytest.raises(H.HadpsgdError):
+        H.Hadpsgd(2, 2, [100, 0])
+    h = H.Hadpsgd(2, 2, [100])
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_weights(2)
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_grads(0, 2)
+    assert h.hadpsgd_launch_count() == 0
+    h.hadpsgd_step(LR, MU, 0)
+    assert h.hadpsgd_launch_count() == 1                         # ONE kernel per step
+    h.close()
+    # arena too small
+    import ctypes
+    from paper_1907_05701_b200 import binding as b
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    opts = b.hadpsgd_opts(small.data_ptr(), 1024, None, 0, 0)
+    arr = (ctypes.c_int64 * 1)(100_000)
+    hh = ctypes.c_void_p()
+    rc = b.lib().hadpsgd_create(2, 2, arr, 1, b.hadpsgd_dtypes(0, 0), ctypes.byref(opts), ctypes.byref(hh))
+    assert rc == b.OUT_OF_MEMORY and not hh
+
+
+# ------------------------------------------------------------------------------- full-size configs
+
+def windows_for(P, seg_len, n_win, width, seed):
+    """Element windows (natural index): the very start, the very end (ragged tail), segment
+    boundaries, and seeded random places."""
+    rng = np.random.default_rng(seed)
+    wins = [(0, width), (P - width, P)]
+    nat = np.concatenate([[0], np.cumsum(seg_len)])
+    for b in nat[1:-1][:: max(1, (len(nat) - 2) // 3)][:3]:
+        wins.append((int(b) - width // 2, int(b) + width // 2))
+    while len(wins) < n_win:
+        lo = int(rng.integers(0, P - width))
+        wins.append((lo, lo + width))
+    return wins[:n_win]
+
+
+def full_size_parity(H, oracle_mod, name, *, exact, n_win=6, width=8192):
+    """BASELINE.json full sizes, in the launch configuration bench.py times (default grid,
+    diagnostics on): run all steps on the GPU with per-step regenerated gradients, then check
+    sampled element windows against the oracle, which re-runs every step on each window with
+    inputs regenerated from (seed, step, s, g, i)."""
+    import torch
+    from fixtures import problem, shapes
+    cfg = shapes.CONFIGS[name]
+    S, G, seg_len, steps = cfg["S"], cfg["G"], cfg["seg_len"], cfg["steps"]
+    bf16 = cfg["grad"] == "bf16"
+    seed = 1000 + len(name)
+    P = int(sum(seg_len))
+    h = H.Hadpsgd(S, G, seg_len, H.BF16 if bf16 else H.F32, H.DETERMINISTIC if exact else 0)
+    problem.fill_weights(h, seed)
+    diags = []
+    for k in range(steps):
+        problem.fill_grads(h, seed, k, cfg["dist"])
+        h.hadpsgd_step(LR, MU, k)
+        diags.append(h.hadpsgd_diagnostics())
+    torch.cuda.synchronize()
+    assert h.hadpsgd_launch_count() == steps
+    for lo, hi in windows_for(P, seg_len, n_win, width, seed):
+        idx = torch.from_numpy(problem.padded_index(seg_len, h.layout["seg_offset"], lo, hi)).cuda()
+        gw = np.stack([h.hadpsgd_weights(s)[idx].cpu().numpy() for s in range(S)])
+        gv = np.stack([h.hadpsgd_momentum(s)[idx].cpu().numpy() for s in range(S)])
+        ow, ov = problem.host_weights(seed, S, lo, hi), np.zeros((S, hi - lo), np.float32)
+        for k in range(steps):
+            oracle_mod.step(problem.host_grads(seed, k, S, G, lo, hi, cfg["dist"], bf16=bf16), ow, ov, LR, MU, k)
+        assert_parity(gw, gv, ow, ov, exact)
+    # properties that hold at any size: both members of the last step's pairs hold the same
+    # bits (R3), and gsq ~ P * sigma^2 / G for i.i.d. gradients of std sigma
+    partner = H.hadpsgd_pairing(S, steps - 1)
+    for s in range(S):
+        if s < partner[s]:
+            assert torch.equal(h.hadpsgd_weights(s), h.hadpsgd_weights(partner[s]))
+    for d in diags:
+        assert np.allclose(d["gsq"], P * 1e-6 / G, rtol=5e-3)
+        assert np.all(d["gap"] > 0) and np.all(d["wsq"] > 0)
+    h.close()
+    torch.cuda.empty_cache()
+
+
+def test_config1_swb300_full_size(H, oracle_mod):
+    """configs[1]: 94,797,312 params flat fp32, S=16, G=4, 20 steps (36.4 GB resident)."""
+    full_size_parity(H, oracle_mod, "swb300", exact=True)
+
+
+def test_config2_swb2000_full_size_exact(H, oracle_mod):
+    """configs[2] (headline): 145,145,344 params flat fp32, S=16, G=4, 20 steps (55.7 GB)."""
+    full_size_parity(H, oracle_mod, "swb2000", exact=True)
+
+
+def test_config2_swb2000_full_size_default_mode(H, oracle_mod):
+    full_size_parity(H, oracle_mod, "swb2000", exact=False, n_win=4)
+
+
+def test_config3_ragged_bf16_full_size(H, oracle_mod):
+    """configs[3]: same 145M shape as a 40-segment ragged table, bf16 grads, S=8, G=8."""
+    full_size_parity(H, oracle_mod, "swb2000_ragged_bf16", exact=True)
+    full_size_parity(H, oracle_mod, "swb2000_ragged_bf16", exact=False, n_win=3)
+
+
+def test_paper_literal_shape(H, oracle_mod):
+    """PAPER.md:106 model (43,130,368 params, '165MB') at 8 super-learners x 8 learners."""
+    full_size_parity(H, oracle_mod, "paper_literal", exact=True, n_win=4)
