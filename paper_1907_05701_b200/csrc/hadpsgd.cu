@@ -46,15 +46,21 @@ static thread_local std::string g_create_error;
 // ---- kernel dispatch -------------------------------------------------------------------
 namespace {
 
-struct LaunchPlan { const void* fn; int threads; };
+struct LaunchPlan { const void* fn; int threads; int tile_units; int blocks_per_sm; };
 
+// Launch shape (profiles/r01_kernel_sweep.md): 256 threads, ONE resident block per SM, and
+// enough 32-byte loads per thread (>= 12) that ~96 KB per SM are in flight.  More resident
+// warps than that measured slower on this path (more DRAM pages open at once).
 template <int G, bool BF16, bool EXACT, bool DIAG, int MODE>
 LaunchPlan plan_for() {
-    // Register budget: 2G+4 (fp32) / 2G+8 (bf16) 16-byte loads are live at once.
-    constexpr int loads = (MODE == kSingle ? 1 : 2) * ((G > 0 ? G : 4) + (BF16 ? 4 : 2));
+    constexpr int members = (MODE == kSingle) ? 1 : 2;
+    constexpr int loads_per_unit = members * ((G > 0 ? G : 4) + (BF16 ? 4 : 2));
+    constexpr int U = loads_per_unit <= 8 ? 2 : 1;
     constexpr int THREADS = 256;
-    constexpr int MINB = loads <= 6 ? 4 : (loads <= 12 ? 3 : (loads <= 20 ? 2 : 1));
-    return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, THREADS, MINB>), THREADS};
+    constexpr int in_flight = THREADS * U * loads_per_unit * 32;           // bytes per block
+    constexpr int BPS = in_flight >= 96 * 1024 ? 1 : (in_flight >= 48 * 1024 ? 2 : 3);
+    return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, U, THREADS, 1>), THREADS,
+            THREADS * U, BPS};
 }
 
 template <int G, bool BF16, bool EXACT, bool DIAG>
@@ -89,7 +95,7 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
     const bool diag = !(h->flags & HADPSGD_NO_DIAG);
     LaunchPlan plan = bf16 ? pick_G<true>(h->L.G, exact, diag, mode) : pick_G<false>(h->L.G, exact, diag, mode);
 
-    const int unit = bf16 ? 8 : 4;
+    const int unit = bf16 ? 16 : 8;   // elements per 32-byte gradient vector
     StepArgs a;
     a.w = reinterpret_cast<float*>(h->arena + h->L.w_off);
     a.v = reinterpret_cast<float*>(h->arena + h->L.v_off);
@@ -109,10 +115,11 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
     int occ = 0;
     CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, 0));
     if (occ < 1) occ = 1;
-    if (h->blocks_per_sm > 0) occ = h->blocks_per_sm;
+    int bps = h->blocks_per_sm > 0 ? h->blocks_per_sm : plan.blocks_per_sm;
+    if (bps > occ) bps = occ;                      // persistent grid: never more than fit at once
     long long n_units = a.unit_end - a.unit_begin;
-    long long want = (n_units + plan.threads - 1) / plan.threads;
-    long long grid = static_cast<long long>(h->num_sms) * occ;
+    long long want = (n_units + plan.tile_units - 1) / plan.tile_units;
+    long long grid = static_cast<long long>(h->num_sms) * bps;
     if (grid > want) grid = want;
     if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;
     if (grid < 1) grid = 1;

@@ -47,13 +47,23 @@ struct StepArgs {
 };
 
 // ---- memory access helpers -------------------------------------------------------------
-// Gradients are touched once per step and never again before they are overwritten:
-// ld.global.cs (evict-first).  w and v are read then rewritten in place; they are also
-// loaded .cs because nothing re-reads them before the whole 55 GB working set has streamed
-// through the 126 MB L2.
-__device__ __forceinline__ float4 ld_stream(const float4* p) { return __ldcs(p); }
-__device__ __forceinline__ uint4 ld_stream(const uint4* p) { return __ldcs(p); }
-__device__ __forceinline__ void st_stream(float4* p, float4 x) { __stcs(p, x); }
+// Every byte is touched once per step, so all traffic is issued as 32-byte vector accesses
+// (ld/st.global.v8.b32, new on sm_100) carrying L2::evict_first: a warp covers 1 KB of each
+// stream per request, which measured ~6 % faster than 16-byte accesses on this path
+// (profiles/r01_kernel_sweep.md) because fewer, longer DRAM bursts are in flight per stream.
+struct Raw8 { unsigned u[8]; };
+__device__ __forceinline__ Raw8 ld_stream32(const void* p) {
+    Raw8 r;
+    asm volatile("ld.global.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r.u[0]), "=r"(r.u[1]), "=r"(r.u[2]), "=r"(r.u[3]), "=r"(r.u[4]), "=r"(r.u[5]), "=r"(r.u[6]), "=r"(r.u[7])
+                 : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream32(void* p, const Raw8& r) {
+    asm volatile("st.global.L1::no_allocate.L2::evict_first.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "l"(p), "r"(r.u[0]), "r"(r.u[1]), "r"(r.u[2]), "r"(r.u[3]), "r"(r.u[4]), "r"(r.u[5]), "r"(r.u[6]), "r"(r.u[7])
+                 : "memory");
+}
 
 template <bool EXACT> __device__ __forceinline__ float add_(float a, float b) { return EXACT ? __fadd_rn(a, b) : a + b; }
 template <bool EXACT> __device__ __forceinline__ float mul_(float a, float b) { return EXACT ? __fmul_rn(a, b) : a * b; }
@@ -66,96 +76,108 @@ template <bool EXACT> __device__ __forceinline__ float wupd_(float lr, float vn,
     return EXACT ? __fsub_rn(w, __fmul_rn(lr, vn)) : fmaf(-lr, vn, w);
 }
 
-// One super-learner's vector unit: UNIT consecutive parameters.
+// One super-learner's vector unit: UNIT consecutive parameters (8 for fp32 gradients, 16 for
+// bf16 gradients, so that a gradient unit is always ONE 32-byte load).
 template <int UNIT> struct Vec { float x[UNIT]; };
 
-// Load + reduce the G learner gradients of super-learner s for one unit (a2).
-// fp32: UNIT = 4, one 16 B load per learner.  bf16: UNIT = 8, one 16 B load per learner,
-// widened exactly (bf16 is the top half of an fp32).
-template <int G, bool BF16, bool EXACT, int UNIT>
-__device__ __forceinline__ void load_grads(const void* gbase, long long P, int Grt, int s,
-                                           long long elem, Vec<UNIT> (&gr)[G > 0 ? G : 1]) {
-    static_assert(G > 0, "templated G only");
+// Widen one 32-byte gradient load to UNIT floats.  bf16 -> fp32 is exact: a bf16 is the top
+// half of an fp32.
+template <bool BF16, int UNIT>
+__device__ __forceinline__ void widen(const Raw8& raw, Vec<UNIT>& out) {
+    if constexpr (BF16) {
 #pragma unroll
-    for (int k = 0; k < G; ++k) {
-        long long off = (static_cast<long long>(s) * Grt + k) * P + elem;
-        if constexpr (BF16) {
-            uint4 raw = ld_stream(reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(gbase) + off));
-            unsigned r[4] = {raw.x, raw.y, raw.z, raw.w};
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                gr[k].x[2 * q] = __uint_as_float(r[q] << 16);
-                gr[k].x[2 * q + 1] = __uint_as_float(r[q] & 0xFFFF0000u);
-            }
-        } else {
-            float4 raw = ld_stream(reinterpret_cast<const float4*>(static_cast<const float*>(gbase) + off));
-            gr[k].x[0] = raw.x; gr[k].x[1] = raw.y; gr[k].x[2] = raw.z; gr[k].x[3] = raw.w;
+        for (int q = 0; q < 8; ++q) {
+            out.x[2 * q] = __uint_as_float(raw.u[q] << 16);
+            out.x[2 * q + 1] = __uint_as_float(raw.u[q] & 0xFFFF0000u);
         }
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) out.x[q] = __uint_as_float(raw.u[q]);
     }
+}
+
+// Issue the G learner-gradient loads of super-learner s for one unit (a2); raw registers.
+template <int G, bool BF16>
+__device__ __forceinline__ void load_grads(const char* gbase, long long P, int s, long long elem, Raw8 (&gr)[G]) {
+    constexpr int EB = BF16 ? 2 : 4;
+#pragma unroll
+    for (int k = 0; k < G; ++k)
+        gr[k] = ld_stream32(gbase + ((static_cast<long long>(s) * G + k) * P + elem) * EB);
 }
 
 template <int UNIT>
 __device__ __forceinline__ void load_state(const float* base, long long off, Vec<UNIT>& out) {
 #pragma unroll
-    for (int q = 0; q < UNIT / 4; ++q) {
-        float4 t = ld_stream(reinterpret_cast<const float4*>(base + off) + q);
-        out.x[4 * q] = t.x; out.x[4 * q + 1] = t.y; out.x[4 * q + 2] = t.z; out.x[4 * q + 3] = t.w;
+    for (int q = 0; q < UNIT / 8; ++q) {
+        Raw8 t = ld_stream32(base + off + 8 * q);
+#pragma unroll
+        for (int e = 0; e < 8; ++e) out.x[8 * q + e] = __uint_as_float(t.u[e]);
     }
 }
 template <int UNIT>
 __device__ __forceinline__ void store_state(float* base, long long off, const Vec<UNIT>& in) {
 #pragma unroll
-    for (int q = 0; q < UNIT / 4; ++q)
-        st_stream(reinterpret_cast<float4*>(base + off) + q,
-                  make_float4(in.x[4 * q], in.x[4 * q + 1], in.x[4 * q + 2], in.x[4 * q + 3]));
-}
-
-// gbar (a2) then v', u (a3) for one super-learner; gradients already in registers.
-template <int G, bool EXACT, int UNIT>
-__device__ __forceinline__ void reduce_update(const Vec<UNIT> (&gr)[G], float invG, float mu, float lr,
-                                              const Vec<UNIT>& w, Vec<UNIT>& v, Vec<UNIT>& u, Vec<UNIT>& gbar) {
+    for (int q = 0; q < UNIT / 8; ++q) {
+        Raw8 t;
 #pragma unroll
-    for (int e = 0; e < UNIT; ++e) {
-        float acc = gr[0].x[e];
-#pragma unroll
-        for (int k = 1; k < G; ++k) acc = add_<EXACT>(acc, gr[k].x[e]);  // fixed learner order g = 0..G-1
-        float gb = mul_<EXACT>(acc, invG);
-        float vn = vupd_<EXACT>(mu, v.x[e], gb);
-        gbar.x[e] = gb;
-        v.x[e] = vn;
-        u.x[e] = wupd_<EXACT>(lr, vn, w.x[e]);
+        for (int e = 0; e < 8; ++e) t.u[e] = __float_as_uint(in.x[8 * q + e]);
+        st_stream32(base + off + 8 * q, t);
     }
 }
 
-// Runtime-G variant (any G >= 1): learners are streamed in batches of 4 loads.
+// Sum of the G learner gradients of one unit, left to right (a2); gradients already in registers.
+template <int G, bool BF16, bool EXACT, int UNIT>
+__device__ __forceinline__ void sum_grads(const Raw8 (&gr)[G], Vec<UNIT>& acc) {
+    widen<BF16, UNIT>(gr[0], acc);
+#pragma unroll
+    for (int k = 1; k < G; ++k) {   // fixed learner order g = 0..G-1
+        Vec<UNIT> t;
+        widen<BF16, UNIT>(gr[k], t);
+#pragma unroll
+        for (int e = 0; e < UNIT; ++e) acc.x[e] = add_<EXACT>(acc.x[e], t.x[e]);
+    }
+}
+
+// Runtime-G sum (any G >= 1): learners are streamed in batches of 4 loads, left to right.
 template <bool BF16, bool EXACT, int UNIT>
-__device__ __forceinline__ void reduce_runtime_G(const void* gbase, long long P, int G, int s, long long elem,
-                                                 Vec<UNIT>& acc) {
-    Vec<UNIT> one[1];
-    load_grads<1, BF16, EXACT, UNIT>(gbase, P, G, s, elem, one);
-    acc = one[0];
+__device__ __forceinline__ void sum_grads_runtime(const char* gbase, long long P, int G, int s, long long elem,
+                                                  Vec<UNIT>& acc) {
+    constexpr int EB = BF16 ? 2 : 4;
+    const char* p0 = gbase + (static_cast<long long>(s) * G * P + elem) * EB;
+    const long long stride = P * EB;
+    widen<BF16, UNIT>(ld_stream32(p0), acc);
     int k = 1;
     for (; k + 4 <= G; k += 4) {
-        Vec<UNIT> b[4];
+        Raw8 b[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) b[j] = ld_stream32(p0 + (k + j) * stride);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            Vec<UNIT> t[1];
-            load_grads<1, BF16, EXACT, UNIT>(static_cast<const char*>(gbase) +
-                                                 static_cast<size_t>(k + j) * P * (BF16 ? 2 : 4),
-                                             P, G, s, elem, t);
-            b[j] = t[0];
+            Vec<UNIT> t;
+            widen<BF16, UNIT>(b[j], t);
+#pragma unroll
+            for (int e = 0; e < UNIT; ++e) acc.x[e] = add_<EXACT>(acc.x[e], t.x[e]);
         }
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-#pragma unroll
-            for (int e = 0; e < UNIT; ++e) acc.x[e] = add_<EXACT>(acc.x[e], b[j].x[e]);
     }
     for (; k < G; ++k) {
-        Vec<UNIT> t[1];
-        load_grads<1, BF16, EXACT, UNIT>(static_cast<const char*>(gbase) + static_cast<size_t>(k) * P * (BF16 ? 2 : 4),
-                                         P, G, s, elem, t);
+        Vec<UNIT> t;
+        widen<BF16, UNIT>(ld_stream32(p0 + k * stride), t);
 #pragma unroll
-        for (int e = 0; e < UNIT; ++e) acc.x[e] = add_<EXACT>(acc.x[e], t[0].x[e]);
+        for (int e = 0; e < UNIT; ++e) acc.x[e] = add_<EXACT>(acc.x[e], t.x[e]);
+    }
+}
+
+// gbar = acc/G (a2), then v' = mu v + gbar, u = w - lr v' (a3).  acc is overwritten by gbar.
+template <bool EXACT, int UNIT>
+__device__ __forceinline__ void apply_update(Vec<UNIT>& acc, float invG, float mu, float lr,
+                                             const Vec<UNIT>& w, Vec<UNIT>& v, Vec<UNIT>& u) {
+#pragma unroll
+    for (int e = 0; e < UNIT; ++e) {
+        float gb = mul_<EXACT>(acc.x[e], invG);
+        float vn = vupd_<EXACT>(mu, v.x[e], gb);
+        acc.x[e] = gb;
+        v.x[e] = vn;
+        u.x[e] = wupd_<EXACT>(lr, vn, w.x[e]);
     }
 }
 
@@ -173,17 +195,20 @@ __device__ __forceinline__ double warp_sum(double x) {
 }
 
 // ---------------------------------------------------------------------------------------
-// The kernel.  G > 0: learner count known at compile time (all gradient loads of a unit are
+// The kernel.  G > 0: learner count known at compile time (all gradient loads of a tile are
 // issued before any is consumed).  G == 0: runtime learner count.
 // Persistent grid: gridDim.x = (#SMs x resident blocks/SM); block b walks tiles b, b+grid, ...
 // of every work item in turn ("pair-major": at any moment the whole chip streams the same
-// 2G+4 read streams and 4 write streams, which keeps DRAM pages open).
+// 2G+4 read streams and 4 write streams, which keeps DRAM pages open).  A tile is
+// THREADS x U units; thread t owns units t, t+THREADS, ... of the tile, so each warp request
+// covers 1 KB contiguous of one stream.
 // ---------------------------------------------------------------------------------------
-template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, int THREADS, int MINB>
+template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, int U, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_constant__ StepArgs a) {
-    constexpr int UNIT = BF16 ? 8 : 4;
+    constexpr int UNIT = BF16 ? 16 : 8;
     constexpr int GA = G > 0 ? G : 1;
     constexpr bool PAIRED = (MODE != kSingle);
+    constexpr int NP = PAIRED ? U : 1;   // array extent of the partner's registers
     __shared__ double s_red[THREADS / 32][kNQ];
     __shared__ unsigned int s_last;
 
@@ -192,76 +217,110 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     const float lr = a.lr, mu = a.mu, invG = a.invG;
     const long long P = a.P;
     const char* gbytes = static_cast<const char*>(a.g);
+    constexpr long long TILE = static_cast<long long>(THREADS) * U;
 
     for (int j = 0; j < a.n_work; ++j) {
         const int s = a.work[j].x, p = a.work[j].y;
         double d_gs = 0., d_gp = 0., d_ws = 0., d_wp = 0., d_gap = 0.;
 
-        for (long long t = static_cast<long long>(blockIdx.x) * THREADS + tid; t < n_units;
-             t += static_cast<long long>(gridDim.x) * THREADS) {
-            const long long elem = (a.unit_begin + t) * UNIT;
-            const long long os = static_cast<long long>(s) * P + elem;
-            const long long op = static_cast<long long>(p) * P + elem;
+        for (long long base = static_cast<long long>(blockIdx.x) * TILE; base < n_units;
+             base += static_cast<long long>(gridDim.x) * TILE) {
+            Vec<UNIT> ws[U], vs[U], gbs[U], wp[NP], vp[NP], gbp[NP];
+            bool live[U];
+            long long elem[U];
+#pragma unroll
+            for (int q = 0; q < U; ++q) {
+                const long long t = base + q * THREADS + tid;
+                live[q] = t < n_units;
+                elem[q] = (a.unit_begin + t) * UNIT;
+            }
 
-            Vec<UNIT> ws, vs, us, gbs, wp, vp, up, gbp;
             if constexpr (G > 0) {
-                // issue every load of the unit first: 2G+4 (fp32) or 2G+8 (bf16) x 16 B in flight
-                Vec<UNIT> grs[GA], grp[GA];
-                load_grads<GA, BF16, EXACT, UNIT>(a.g, P, G, s, elem, grs);
-                if constexpr (PAIRED) load_grads<GA, BF16, EXACT, UNIT>(a.g, P, G, p, elem, grp);
-                load_state<UNIT>(a.w, os, ws);
-                load_state<UNIT>(a.v, os, vs);
-                if constexpr (PAIRED) { load_state<UNIT>(a.w, op, wp); load_state<UNIT>(a.v, op, vp); }
-                reduce_update<GA, EXACT, UNIT>(grs, invG, mu, lr, ws, vs, us, gbs);
-                if constexpr (PAIRED) reduce_update<GA, EXACT, UNIT>(grp, invG, mu, lr, wp, vp, up, gbp);
+                // issue every load of the tile first: U x (2G + 4 x UNIT/8) x 32 B in flight per thread
+                Raw8 grs[U][GA], grp[NP][GA];
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    if (live[q]) {
+                        load_grads<GA, BF16>(gbytes, P, s, elem[q], grs[q]);
+                        if constexpr (PAIRED) load_grads<GA, BF16>(gbytes, P, p, elem[q], grp[q]);
+                        load_state<UNIT>(a.w, static_cast<long long>(s) * P + elem[q], ws[q]);
+                        load_state<UNIT>(a.v, static_cast<long long>(s) * P + elem[q], vs[q]);
+                        if constexpr (PAIRED) {
+                            load_state<UNIT>(a.w, static_cast<long long>(p) * P + elem[q], wp[q]);
+                            load_state<UNIT>(a.v, static_cast<long long>(p) * P + elem[q], vp[q]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    if (live[q]) {
+                        sum_grads<GA, BF16, EXACT, UNIT>(grs[q], gbs[q]);
+                        if constexpr (PAIRED) sum_grads<GA, BF16, EXACT, UNIT>(grp[q], gbp[q]);
+                    }
+                }
             } else {
-                load_state<UNIT>(a.w, os, ws);
-                load_state<UNIT>(a.v, os, vs);
-                if constexpr (PAIRED) { load_state<UNIT>(a.w, op, wp); load_state<UNIT>(a.v, op, vp); }
-                Vec<UNIT> acc[1];
-                reduce_runtime_G<BF16, EXACT, UNIT>(gbytes, P, a.G, s, elem, acc[0]);
-                reduce_update<1, EXACT, UNIT>(acc, invG, mu, lr, ws, vs, us, gbs);
-                if constexpr (PAIRED) {
-                    reduce_runtime_G<BF16, EXACT, UNIT>(gbytes, P, a.G, p, elem, acc[0]);
-                    reduce_update<1, EXACT, UNIT>(acc, invG, mu, lr, wp, vp, up, gbp);
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    if (live[q]) {
+                        load_state<UNIT>(a.w, static_cast<long long>(s) * P + elem[q], ws[q]);
+                        load_state<UNIT>(a.v, static_cast<long long>(s) * P + elem[q], vs[q]);
+                        if constexpr (PAIRED) {
+                            load_state<UNIT>(a.w, static_cast<long long>(p) * P + elem[q], wp[q]);
+                            load_state<UNIT>(a.v, static_cast<long long>(p) * P + elem[q], vp[q]);
+                        }
+                        sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, s, elem[q], gbs[q]);
+                        if constexpr (PAIRED) sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, p, elem[q], gbp[q]);
+                    }
                 }
             }
 
-            // a4: pairwise average.  Default (R3): both members get 1/2 (u_s + u_p).
-            // kPairEq7: eq. (7) as printed, w'_s = 1/2 (w_s + w_p) - lr v'_s.
-            Vec<UNIT> outs, outp, dif;
-            if constexpr (MODE == kPair) {
 #pragma unroll
-                for (int e = 0; e < UNIT; ++e) {
-                    float m = mul_<EXACT>(0.5f, add_<EXACT>(us.x[e], up.x[e]));
-                    outs.x[e] = m; outp.x[e] = m;
-                    if constexpr (DIAG) dif.x[e] = us.x[e] - up.x[e];
-                }
-            } else if constexpr (MODE == kPairEq7) {
+            for (int q = 0; q < U; ++q) {
+                if (!live[q]) continue;
+                const long long os = static_cast<long long>(s) * P + elem[q];
+                const long long op = static_cast<long long>(p) * P + elem[q];
+                Vec<UNIT> us, up, outs, outp, dif;
+                apply_update<EXACT, UNIT>(gbs[q], invG, mu, lr, ws[q], vs[q], us);
+                if constexpr (PAIRED) apply_update<EXACT, UNIT>(gbp[q], invG, mu, lr, wp[q], vp[q], up);
+
+                // a4: pairwise average.  Default (R3): both members get 1/2 (u_s + u_p).
+                // kPairEq7: eq. (7) as printed, w'_s = 1/2 (w_s + w_p) - lr v'_s.
+                if constexpr (MODE == kPair) {
 #pragma unroll
-                for (int e = 0; e < UNIT; ++e) {
-                    float m = mul_<EXACT>(0.5f, add_<EXACT>(ws.x[e], wp.x[e]));
-                    // u = w - lr v' was formed above; recover lr v' the same way the oracle does
-                    float ts = mul_<EXACT>(lr, vs.x[e]), tp = mul_<EXACT>(lr, vp.x[e]);
-                    outs.x[e] = EXACT ? __fsub_rn(m, ts) : m - ts;
-                    outp.x[e] = EXACT ? __fsub_rn(m, tp) : m - tp;
-                    if constexpr (DIAG) dif.x[e] = ws.x[e] - wp.x[e];
+                    for (int e = 0; e < UNIT; ++e) {
+                        float m = mul_<EXACT>(0.5f, add_<EXACT>(us.x[e], up.x[e]));
+                        outs.x[e] = m;
+                        if constexpr (DIAG) dif.x[e] = us.x[e] - up.x[e];
+                    }
+                } else if constexpr (MODE == kPairEq7) {
+#pragma unroll
+                    for (int e = 0; e < UNIT; ++e) {
+                        float m = mul_<EXACT>(0.5f, add_<EXACT>(ws[q].x[e], wp[q].x[e]));
+                        // recover lr v' the same way the oracle does (one fp32 multiply)
+                        float ts = mul_<EXACT>(lr, vs[q].x[e]), tp = mul_<EXACT>(lr, vp[q].x[e]);
+                        outs.x[e] = EXACT ? __fsub_rn(m, ts) : m - ts;
+                        outp.x[e] = EXACT ? __fsub_rn(m, tp) : m - tp;
+                        if constexpr (DIAG) dif.x[e] = ws[q].x[e] - wp[q].x[e];
+                    }
+                } else {
+                    outs = us;
                 }
-            } else {
-                outs = us;
-            }
 
-            store_state<UNIT>(a.v, os, vs);
-            store_state<UNIT>(a.w, os, outs);
-            if constexpr (PAIRED) { store_state<UNIT>(a.v, op, vp); store_state<UNIT>(a.w, op, outp); }
-
-            if constexpr (DIAG) {
-                d_gs += static_cast<double>(sumsq<UNIT>(gbs));
-                d_ws += static_cast<double>(sumsq<UNIT>(outs));
+                store_state<UNIT>(a.v, os, vs[q]);
+                store_state<UNIT>(a.w, os, outs);
                 if constexpr (PAIRED) {
-                    d_gp += static_cast<double>(sumsq<UNIT>(gbp));
-                    d_gap += static_cast<double>(sumsq<UNIT>(dif));
-                    if constexpr (MODE == kPairEq7) d_wp += static_cast<double>(sumsq<UNIT>(outp));
+                    store_state<UNIT>(a.v, op, vp[q]);
+                    store_state<UNIT>(a.w, op, MODE == kPair ? outs : outp);
+                }
+
+                if constexpr (DIAG) {
+                    d_gs += static_cast<double>(sumsq<UNIT>(gbs[q]));
+                    d_ws += static_cast<double>(sumsq<UNIT>(outs));
+                    if constexpr (PAIRED) {
+                        d_gp += static_cast<double>(sumsq<UNIT>(gbp[q]));
+                        d_gap += static_cast<double>(sumsq<UNIT>(dif));
+                        if constexpr (MODE == kPairEq7) d_wp += static_cast<double>(sumsq<UNIT>(outp));
+                    }
                 }
             }
         }
