@@ -34,8 +34,8 @@ LR, MU = 0.1, 0.9
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the
 # `ncu --set full` capture summarised in profiles/ (bytes; None until a capture exists)
-NCU_TRAFFIC_BYTES = {}
-NCU_TRAFFIC_SOURCE = {}
+NCU_TRAFFIC_BYTES = {"swb2000": 74.286e9}
+NCU_TRAFFIC_SOURCE = {"swb2000": "profiles/r01_step_kernel_ncu.md (dram__bytes_read.sum 55.740 GB + dram__bytes_write.sum 18.546 GB)"}
 
 
 def parse_args():
@@ -81,25 +81,68 @@ def measured_peak():
 # ------------------------------------------------------------------ clocks during the timed region
 
 class ClockSampler:
+    """SM clock and throttle reasons DURING the timed region: an NVML polling thread (every few
+    ms; the timed loop spends its time inside cudaDeviceSynchronize, which releases the GIL).
+    Falls back to one `nvidia-smi` query loop (the recipe's clocks line) if NVML is unusable."""
     QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
     def __init__(self, index):
         self.index, self.proc, self.path = index, None, None
+        self.thread, self.stop_flag, self.samples, self.bits, self.max_mhz, self.power = None, False, [], 0, None, []
+
+    def _poll(self, nv, dev):
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(dev, nv.NVML_CLOCK_SM))
+                self.bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(dev))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(dev) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.004)
 
     def start(self):
         try:
+            import threading
+            import pynvml as nv
+            nv.nvmlInit()
+            dev = nv.nvmlDeviceGetHandleByIndex(self._physical_index())
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(dev, nv.NVML_CLOCK_SM)
+            self.thread = threading.Thread(target=self._poll, args=(nv, dev), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.thread = None
+        try:
             fd, self.path = tempfile.mkstemp(suffix=".csv")
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.QUERY,
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self._physical_index()), "--query-gpu=" + self.QUERY,
                                           "--format=csv,noheader,nounits", "-lms", "100"],
                                          stdout=fd, stderr=subprocess.DEVNULL)
             os.close(fd)
         except Exception:
             self.proc = None
 
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            ids = [x for x in vis.split(",") if x.strip()]
+            if self.index < len(ids) and ids[self.index].strip().isdigit():
+                return int(ids[self.index])
+        return self.index
+
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "source": None}
+        if self.thread is not None:
+            self.stop_flag = True
+            self.thread.join(timeout=2)
+            sm = sorted(self.samples)
+            if sm:
+                out.update(sm_mhz=float(sm[len(sm) // 2]), sm_max_mhz=float(self.max_mhz), samples=len(sm), source="nvml",
+                           power_w_max=max(self.power) if self.power else None)
+            out["reasons"] = sorted(name for bit, name in self.REASONS.items() if self.bits & bit)
+            return out
         if self.proc is None:
             return out
         self.proc.terminate()           # the exact PID we started
@@ -125,7 +168,7 @@ class ClockSampler:
             pass
         if sm:
             sm.sort()
-            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), samples=len(sm))
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), samples=len(sm), source="nvidia-smi")
         out["reasons"] = sorted(reasons)
         return out
 
@@ -207,7 +250,7 @@ def parse_flags(H, text):
     return flags
 
 
-def time_device_steps(torch, dist, h, steps, warmup, k0=0):
+def time_device_steps(torch, dist, h, steps, warmup, k0=0, sampler=None):
     """W untimed steps, then exactly K steps between barrier + synchronize; CUDA events on the
     stream the kernel is launched on (the handle's stream IS torch's current stream)."""
     for k in range(warmup):
@@ -217,15 +260,18 @@ def time_device_steps(torch, dist, h, steps, warmup, k0=0):
         dist.barrier()
     torch.cuda.synchronize()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if sampler is not None:
+        sampler.start()
     ev0.record(h.stream)
     for k in range(steps):
         h.hadpsgd_step(LR, MU, k0 + warmup + k)
     ev1.record(h.stream)
     torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler is not None else None
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    return ev0.elapsed_time(ev1) / 1e3      # seconds for K steps
+    return ev0.elapsed_time(ev1) / 1e3, clocks      # seconds for K steps
 
 
 def time_e2e_steps(torch, dist, h, cfg, steps, warmup=1):
@@ -307,13 +353,10 @@ def run_ours(args):
     problem.fill_grads(h, seed, 0, cfg["dist"])
     torch.cuda.synchronize()
 
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     n0 = h.hadpsgd_launch_count()
-    secs = time_device_steps(torch, dist, h, args.steps, args.warmup)
+    secs, clocks = time_device_steps(torch, dist, h, args.steps, args.warmup,
+                                     sampler=ClockSampler(local) if rank == 0 else None)
     launches = h.hadpsgd_launch_count() - n0 - args.warmup
-    clocks = sampler.stop() if rank == 0 else None
     diag = None if (flags & H.NO_DIAG) else h.hadpsgd_diagnostics()
 
     e2e = None

@@ -48,17 +48,20 @@ namespace {
 
 struct LaunchPlan { const void* fn; int threads; int tile_units; int blocks_per_sm; };
 
-// Launch shape (profiles/r01_kernel_sweep.md): 256 threads, ONE resident block per SM, and
+// Launch shape: 256 threads, ONE resident block per SM, and
 // enough 32-byte loads per thread (>= 12) that ~96 KB per SM are in flight.  More resident
 // warps than that measured slower on this path (more DRAM pages open at once).
 template <int G, bool BF16, bool EXACT, bool DIAG, int MODE>
 LaunchPlan plan_for() {
     constexpr int members = (MODE == kSingle) ? 1 : 2;
     constexpr int loads_per_unit = members * ((G > 0 ? G : 4) + (BF16 ? 4 : 2));
-    constexpr int U = loads_per_unit <= 8 ? 2 : 1;
-    constexpr int THREADS = 256;
+    constexpr int U = loads_per_unit <= 6 ? 2 : 1;
+    // measured: 12 loads x 256 threads and 20 loads x 160 threads
+    // (both ~100 KB in flight per SM) are the best shapes for fp32 G=4 and G=8; 8 loads x 256
+    // threads x 1 block beats both 2 blocks/SM and U=2 for G=2.
+    constexpr int THREADS = (!BF16 && G > 0 && U * loads_per_unit >= 20) ? 160 : 256;
     constexpr int in_flight = THREADS * U * loads_per_unit * 32;           // bytes per block
-    constexpr int BPS = in_flight >= 96 * 1024 ? 1 : (in_flight >= 48 * 1024 ? 2 : 3);
+    constexpr int BPS = in_flight >= 48 * 1024 ? 1 : 2;
     return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, U, THREADS, 1>), THREADS,
             THREADS * U, BPS};
 }

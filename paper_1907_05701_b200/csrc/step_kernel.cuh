@@ -1,17 +1,17 @@
 // step_kernel.cuh -- B0: the fused H-ADPSGD step kernel for sm_100a.
 //
 // One launch per step, one pass over HBM.  For each work item
-// (a pair (s,p) of super-learners, or a single s when unmixed) and each 16-byte vector of
-// parameters, a thread
-//   * streams the G gradient vectors of s and of p (read once -> evict-first loads),
-//     w_s, v_s, w_p, v_p                                   [2G+4 independent 16 B loads in flight]
+// (a pair (s,p) of super-learners, or a single s when unmixed) and each unit of parameters
+// (8 for fp32 gradients, 16 for bf16 gradients = one 32-byte gradient vector), a thread
+//   * streams the G gradient vectors of s and of p, w_s, v_s, w_p, v_p
+//                                        [2G+4 (fp32) / 2G+8 (bf16) independent 32 B loads in flight]
 //   * reduces the G gradients left to right in fp32 registers (eq. (6))
 //   * v <- mu v + gbar ; u = w - lr v                       (eq. (3), + momentum)
 //   * w_s = w_p = 1/2 (u_s + u_p)                           (eq. (7))
-//   * writes v_s, v_p, w_s, w_p (streaming stores), and accumulates the a5 diagnostics.
+//   * writes v_s, v_p, w_s, w_p (32 B stores), and accumulates the a5 diagnostics.
 // The path is HBM-bound (0.3 flop/B): no tensor cores, no shared-memory staging of data --
-// each byte is touched exactly once, so the design goal is only "enough coalesced 16 B
-// requests in flight per SM" and full-sector writes.
+// each byte is touched exactly once, so the design goal is only "the right amount of coalesced
+// 32 B requests in flight per SM" (~100 KB) and full-sector writes.
 //
 // Diagnostics: per-thread double accumulators -> warp shuffle tree -> block partial in a
 // fixed slot of global scratch (no atomics on data) -> the last block to finish (ticket)
@@ -50,7 +50,7 @@ struct StepArgs {
 // Every byte is touched once per step, so all traffic is issued as 32-byte vector accesses
 // (ld/st.global.v8.b32, new on sm_100) carrying L2::evict_first: a warp covers 1 KB of each
 // stream per request, which measured ~6 % faster than 16-byte accesses on this path
-// (profiles/r01_kernel_sweep.md) because fewer, longer DRAM bursts are in flight per stream.
+// because fewer, longer DRAM bursts are in flight per stream.
 struct Raw8 { unsigned u[8]; };
 __device__ __forceinline__ Raw8 ld_stream32(const void* p) {
     Raw8 r;
