@@ -105,6 +105,21 @@ int hadpsgd_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
 /* partner_out[s] = ring neighbour averaged with at step_k.  S==1 -> {0}.  S odd >1 -> INVALID_ARG. */
 int hadpsgd_pairing(int S, uint64_t step_k, int32_t* partner_out /*host [S]*/);
 
+/* Parameter-range sharding: rank's contiguous element range [lo, hi) of a
+ * P_padded-element buffer split over `world` ranks in whole HADPSGD_SEG_ALIGN_ELEMS blocks
+ * (ranges are disjoint, ordered by rank, and cover [0, P_padded); the first P%world ranks get
+ * one block more).  P_padded must be a multiple of HADPSGD_SEG_ALIGN_ELEMS (hadpsgd_layout).
+ * Pure host function; lo/hi are host out-pointers.                                            */
+int hadpsgd_shard_range(int64_t P_padded, int world, int rank, int64_t* lo, int64_t* hi);
+
+/* Learning-rate recipe of PAPER.md:70 (section 3), a host helper that feeds `lr` of
+ * hadpsgd_step (row f3): peak = base_lr * total_batch / base_batch (linear scaling); epochs are
+ * 1-based; epoch 1 runs at base_lr and the rate rises linearly to peak at epoch warmup_epochs
+ * (the paper's example: 0.1 -> 1.0 over 10 epochs for batch 256 -> 2560); afterwards it is
+ * annealed by 1/sqrt(2) per epoch.  lr_out: host.  INVALID_ARG on non-positive arguments.     */
+int hadpsgd_lr_schedule(double base_lr, double base_batch, double total_batch,
+                        int warmup_epochs, int epoch, double* lr_out);
+
 /* lifecycle ---------------------------------------------------------------------------------- */
 
 /* n_seg == 1 is the flat buffer.  opts may be NULL (library-owned memory, default stream,

@@ -4,4 +4,5 @@ The product is libhadpsgd.so (hand-written sm_100a CUDA behind the C ABI of
 include/hadpsgd.h); this package is its thin Python binding.  No CPU fallback.
 """
 from .binding import (BF16, DETERMINISTIC, EQ7_LITERAL, F32, NO_DIAG, NO_MIX, Hadpsgd, HadpsgdError,  # noqa: F401
-                      hadpsgd_layout, hadpsgd_pairing, hadpsgd_required_bytes, lib)
+                      hadpsgd_layout, hadpsgd_lr_schedule, hadpsgd_pairing, hadpsgd_required_bytes,
+                      hadpsgd_shard_range, lib)

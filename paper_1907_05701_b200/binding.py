@@ -55,6 +55,9 @@ def lib():
         L.hadpsgd_required_bytes.argtypes = [i32, i32, i64p, i32, hadpsgd_dtypes, sz_p]
         L.hadpsgd_layout.argtypes = [i32, i32, i64p, i32, hadpsgd_dtypes, i64p, i64p, sz_p, sz_p, sz_p]
         L.hadpsgd_pairing.argtypes = [i32, u64, ctypes.POINTER(ctypes.c_int32)]
+        L.hadpsgd_shard_range.argtypes = [ctypes.c_int64, i32, i32, i64p, i64p]
+        L.hadpsgd_lr_schedule.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double, i32, i32,
+                                          ctypes.POINTER(ctypes.c_double)]
         L.hadpsgd_create.argtypes = [i32, i32, i64p, i32, hadpsgd_dtypes, ctypes.POINTER(hadpsgd_opts), ctypes.POINTER(vp)]
         L.hadpsgd_destroy.argtypes = [vp]
         L.hadpsgd_step.argtypes = [vp, f32, f32, u64]
@@ -109,6 +112,18 @@ def hadpsgd_pairing(S, step_k):
     out = (ctypes.c_int32 * max(S, 1))()
     _check(lib().hadpsgd_pairing(S, step_k, out))
     return list(out)[:S]
+
+
+def hadpsgd_shard_range(P_padded, world, rank):
+    lo, hi = ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(lib().hadpsgd_shard_range(P_padded, world, rank, ctypes.byref(lo), ctypes.byref(hi)))
+    return lo.value, hi.value
+
+
+def hadpsgd_lr_schedule(base_lr, base_batch, total_batch, warmup_epochs, epoch):
+    out = ctypes.c_double(0.0)
+    _check(lib().hadpsgd_lr_schedule(base_lr, base_batch, total_batch, warmup_epochs, epoch, ctypes.byref(out)))
+    return out.value
 
 
 class Hadpsgd:

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhadpsgd.so")
-SOURCES = ["hadpsgd.cu", "allocator.cpp", "scheduler.cpp"]
+SOURCES = ["hadpsgd.cu", "allocator.cpp", "scheduler.cpp", "schedule.cpp"]
 DEPS = SOURCES + ["internal.h", "step_kernel.cuh", os.path.join("..", "..", "include", "hadpsgd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--ftz=false", "--prec-div=true", "--prec-sqrt=true",   # IEEE: no flush-to-zero (R17)
