@@ -53,6 +53,9 @@ def parse_args():
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE.json configs[4]: bandwidth sweep over P, S, G (one JSON line per point)")
+    ap.add_argument("--sweep-md", default="", help="also write the sweep as a markdown table to this path")
     return ap.parse_args()
 
 
@@ -366,14 +369,13 @@ def run_ours(args):
 
     # max over ranks (device time), diagnostics summed over the parameter shards
     if dist is not None:
-        t = torch.tensor([secs, e2e[0] if e2e else 0.0], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        secs = float(t[0])
+        from paper_1907_05701_b200 import sharding
+        secs = sharding.max_over_ranks(secs, dist, "cuda")
         if e2e:
-            e2e = (float(t[1]),) + e2e[1:]
+            e2e = (sharding.max_over_ranks(e2e[0], dist, "cuda"),) + e2e[1:]
         if diag is not None:
-            dsum = torch.tensor(list(diag["gsq"]) + list(diag["wsq"]) + list(diag["gap"]), dtype=torch.float64, device="cuda")
-            dist.all_reduce(dsum)             # the only collective: 3*S doubles, outside the timed region
+            # the only collective: 3*S doubles, outside the timed region
+            diag = sharding.allreduce_diagnostics(diag, dist, "cuda")
     h.close()
 
     if rank == 0:
@@ -409,9 +411,53 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: flat fp32 buffer of 2^10..2^28 params (powers of 4), G in {2,4,8},
+    S in {2,4,8,16} with S*G*P*4 B <= 96 GB; uniform grads in [-1e-3, 1e-3]; W warm + K timed steps
+    per point (defaults 5 + 20); GB/s (algorithmic) vs buffer size.  Small points are L2-resident
+    (working set < 126 MB) and launch-latency bound: they are flagged, not bandwidth claims."""
+    import torch
+    import paper_1907_05701_b200 as H
+    from fixtures import problem, shapes
+    H.lib()
+    torch.cuda.set_device(0)
+    peak, peak_src = measured_peak()
+    rows = []
+    for P, S, G in shapes.sweep_points():
+        h = H.Hadpsgd(S, G, [P], H.F32, parse_flags(H, args.flags), device=0)
+        problem.fill_weights(h, 3000)
+        problem.fill_grads(h, 3000, 0, "uniform")
+        torch.cuda.synchronize()
+        secs, _ = time_device_steps(torch, None, h, args.steps, args.warmup)
+        t = secs / args.steps
+        cfg = {"S": S, "G": G, "P": P, "b_g": 4}
+        row = {"P": P, "S": S, "G": G, "us_per_step": t * 1e6, "gb_per_s": algorithmic_bytes(cfg) / t / 1e9,
+               "learner_params_per_s": S * G * P / t, "resident_bytes": h.arena_bytes,
+               "l2_resident": h.arena_bytes < 126e6}
+        row["frac_of_measured_peak"] = row["gb_per_s"] / peak
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+        h.close()
+        del h
+        torch.cuda.empty_cache()
+    if args.sweep_md:
+        with open(args.sweep_md, "w") as f:
+            f.write(f"# Bandwidth sweep (BASELINE.json configs[4])\n\nCommand: `python bench.py --sweep --steps {args.steps} "
+                    f"--warmup {args.warmup} --sweep-md {args.sweep_md}`; flat fp32, uniform gradients, diagnostics on; "
+                    f"GB/s = S*P*(4G+16) / t_step; peak = {peak} GB/s ({peak_src}).  Points whose resident set is below the "
+                    "126 MB L2 are marked L2: their GB/s is cache bandwidth or launch latency, not HBM.\n\n")
+            f.write("| P | S | G | resident MB | us/step | GB/s | of peak | |\n|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write(f"| 2^{r['P'].bit_length() - 1} | {r['S']} | {r['G']} | {r['resident_bytes'] / 1e6:.1f} | "
+                        f"{r['us_per_step']:.2f} | {r['gb_per_s']:.1f} | {r['frac_of_measured_peak']:.3f} | "
+                        f"{'L2' if r['l2_resident'] else ''} |\n")
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -121,7 +121,7 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
     int bps = h->blocks_per_sm > 0 ? h->blocks_per_sm : plan.blocks_per_sm;
     if (bps > occ) bps = occ;                      // persistent grid: never more than fit at once
     long long n_units = a.unit_end - a.unit_begin;
-    long long want = (n_units + plan.tile_units - 1) / plan.tile_units;
+    long long want = (n_units + plan.tile_units - 1) / plan.tile_units * a.n_work;   // (item, tile) pairs
     long long grid = static_cast<long long>(h->num_sms) * bps;
     if (grid > want) grid = want;
     if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;

@@ -197,9 +197,10 @@ __device__ __forceinline__ double warp_sum(double x) {
 // ---------------------------------------------------------------------------------------
 // The kernel.  G > 0: learner count known at compile time (all gradient loads of a tile are
 // issued before any is consumed).  G == 0: runtime learner count.
-// Persistent grid: gridDim.x = (#SMs x resident blocks/SM); block b walks tiles b, b+grid, ...
-// of every work item in turn ("pair-major": at any moment the whole chip streams the same
-// 2G+4 read streams and 4 write streams, which keeps DRAM pages open).  A tile is
+// Persistent grid: gridDim.x = (#SMs x resident blocks/SM); block b walks global tiles b,
+// b+grid, ... of the item-major (work item, tile) space ("pair-major": for large P the whole
+// chip streams the same 2G+4 read streams and 4 write streams at any moment, which keeps DRAM
+// pages open; for small P the items spread over the blocks instead of serialising).  A tile is
 // THREADS x U units; thread t owns units t, t+THREADS, ... of the tile, so each warp request
 // covers 1 KB contiguous of one stream.
 // ---------------------------------------------------------------------------------------
@@ -219,12 +220,46 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     const char* gbytes = static_cast<const char*>(a.g);
     constexpr long long TILE = static_cast<long long>(THREADS) * U;
 
-    for (int j = 0; j < a.n_work; ++j) {
-        const int s = a.work[j].x, p = a.work[j].y;
-        double d_gs = 0., d_gp = 0., d_ws = 0., d_wp = 0., d_gap = 0.;
+    // a5: flush this block's partial sums of work item j to its fixed slot partials[j][q][block]
+    double d_gs = 0., d_gp = 0., d_ws = 0., d_wp = 0., d_gap = 0.;
+    auto flush = [&](int j) {
+        if constexpr (MODE == kPair) d_wp = d_ws;
+        double q[kNQ] = {d_gs, d_gp, d_ws, d_wp, d_gap};
+#pragma unroll
+        for (int k = 0; k < kNQ; ++k) q[k] = warp_sum(q[k]);
+        if ((tid & 31) == 0)
+#pragma unroll
+            for (int k = 0; k < kNQ; ++k) s_red[tid >> 5][k] = q[k];
+        __syncthreads();
+        if (tid < kNQ) {
+            double tot = 0.;
+            for (int wi = 0; wi < THREADS / 32; ++wi) tot += s_red[wi][tid];  // fixed order
+            a.partials[(static_cast<size_t>(j) * kNQ + tid) * gridDim.x + blockIdx.x] = tot;
+        }
+        __syncthreads();
+        d_gs = d_gp = d_ws = d_wp = d_gap = 0.;
+    };
+    if constexpr (DIAG) {
+        // slots of work items this block never touches (small problems) must read as zero
+        for (int idx = tid; idx < a.n_work * kNQ; idx += THREADS)
+            a.partials[static_cast<size_t>(idx) * gridDim.x + blockIdx.x] = 0.;
+        __syncthreads();
+    }
 
-        for (long long base = static_cast<long long>(blockIdx.x) * TILE; base < n_units;
-             base += static_cast<long long>(gridDim.x) * TILE) {
+    // Flattened (work item, tile) space, item-major: block b takes global tiles b, b+grid, ...
+    // For large P every block walks all items in order (the whole chip streams one pair at a
+    // time); for small P the items spread over the blocks instead of serialising.
+    const long long n_tiles = (n_units + TILE - 1) / TILE;
+    const long long total_tiles = n_tiles * a.n_work;
+    int cur = -1, s = 0, p = 0;
+    for (long long gt = blockIdx.x; gt < total_tiles; gt += gridDim.x) {
+        const int j = static_cast<int>(gt / n_tiles);
+        const long long base = (gt - static_cast<long long>(j) * n_tiles) * TILE;
+        if (j != cur) {                       // block-uniform: every thread sees the same gt
+            if constexpr (DIAG) { if (cur >= 0) flush(cur); }
+            cur = j; s = a.work[j].x; p = a.work[j].y;
+        }
+        {
             Vec<UNIT> ws[U], vs[U], gbs[U], wp[NP], vp[NP], gbp[NP];
             bool live[U];
             long long elem[U];
@@ -325,24 +360,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             }
         }
 
-        if constexpr (DIAG) {
-            if constexpr (MODE == kPair) d_wp = d_ws;
-            // block partial for work item j -> partials[j][q][blockIdx.x]
-            double q[kNQ] = {d_gs, d_gp, d_ws, d_wp, d_gap};
-#pragma unroll
-            for (int k = 0; k < kNQ; ++k) q[k] = warp_sum(q[k]);
-            if ((tid & 31) == 0)
-#pragma unroll
-                for (int k = 0; k < kNQ; ++k) s_red[tid >> 5][k] = q[k];
-            __syncthreads();
-            if (tid < kNQ) {
-                double tot = 0.;
-                for (int wi = 0; wi < THREADS / 32; ++wi) tot += s_red[wi][tid];  // fixed order
-                a.partials[(static_cast<size_t>(j) * kNQ + tid) * gridDim.x + blockIdx.x] = tot;
-            }
-            __syncthreads();
-        }
     }
+    if constexpr (DIAG) { if (cur >= 0) flush(cur); }
 
     if constexpr (DIAG) {
         // last block to arrive reduces all block partials in a fixed order
