@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "internal.h"
@@ -20,6 +21,7 @@ struct hadpsgd_ctx {
     cudaStream_t stream = nullptr;
     cudaStream_t copy_stream = nullptr;   // host path: H2D copies overlap the kernel
     std::vector<cudaEvent_t> chunk_events;
+    std::vector<std::pair<const void*, int>> occupancy;   // per kernel instantiation, queried once
     char* arena = nullptr;
     bool owns_arena = false;
     double* d_partials = nullptr;
@@ -116,8 +118,12 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
     for (size_t j = 0; j < items.size(); ++j) a.work[j] = make_short2(static_cast<short>(items[j].a), static_cast<short>(items[j].b));
 
     int occ = 0;
-    CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, 0));
-    if (occ < 1) occ = 1;
+    for (const auto& kv : h->occupancy) if (kv.first == plan.fn) occ = kv.second;
+    if (occ == 0) {
+        CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, 0));
+        if (occ < 1) occ = 1;
+        h->occupancy.emplace_back(plan.fn, occ);
+    }
     int bps = h->blocks_per_sm > 0 ? h->blocks_per_sm : plan.blocks_per_sm;
     if (bps > occ) bps = occ;                      // persistent grid: never more than fit at once
     long long n_units = a.unit_end - a.unit_begin;

@@ -298,6 +298,38 @@ def test_error_codes(H, torch_cuda):
     assert rc == b.OUT_OF_MEMORY and not hh
 
 
+def test_cuda_graph_capture_and_replay(H, oracle_mod, torch_cuda):
+    """hadpsgd_step only enqueues on its stream, so an (even, odd) step pair can be captured into a
+    CUDA graph and replayed; 3 replays = 6 steps must equal 6 oracle steps bit for bit."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed = 4, 2, 123_457, 101
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC, stream=side)
+        problem.fill_weights(h, seed)
+        problem.fill_grads(h, seed, 0)
+    side.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        h.hadpsgd_step(LR, MU, 0)
+        h.hadpsgd_step(LR, MU, 1)
+    assert h.hadpsgd_launch_count() == 2
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    og = problem.host_grads(seed, 0, S, G, 0, P)
+    for k in range(6):
+        oracle_mod.step(og, ow, ov, LR, MU, k)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    assert_parity(gw, gv, ow, ov, True)
+    d = h.hadpsgd_diagnostics()
+    assert d["step_k"] == 1 and np.all(d["gsq"] > 0)
+    h.close()
+
+
 # ------------------------------------------------------------------------------- full-size configs
 
 def windows_for(P, seg_len, n_win, width, seed):
@@ -374,6 +406,31 @@ def test_config3_ragged_bf16_full_size(H, oracle_mod):
     """configs[3]: same 145M shape as a 40-segment ragged table, bf16 grads, S=8, G=8."""
     full_size_parity(H, oracle_mod, "swb2000_ragged_bf16", exact=True)
     full_size_parity(H, oracle_mod, "swb2000_ragged_bf16", exact=False, n_win=3)
+
+
+def test_largest_sweep_point_windows(H, oracle_mod, torch_cuda):
+    """configs[4] at its maximum size: flat fp32 2^28 params, S=16, G=4 (103 GB resident; byte
+    offsets up to 2^36), uniform gradients, 3 steps; sampled windows against the oracle."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed, steps = 16, 4, 1 << 28, 77, 3
+    free, _ = torch.cuda.mem_get_info()
+    assert free > H.hadpsgd_required_bytes(S, G, [P]), "needs ~103 GB of free HBM"
+    h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
+    problem.fill_weights(h, seed)
+    for k in range(steps):
+        problem.fill_grads(h, seed, k, "uniform")
+        h.hadpsgd_step(LR, MU, k)
+    torch.cuda.synchronize()
+    for lo, hi in windows_for(P, [P], 5, 4096, seed):
+        gw = np.stack([h.hadpsgd_weights(s)[lo:hi].cpu().numpy() for s in range(S)])
+        gv = np.stack([h.hadpsgd_momentum(s)[lo:hi].cpu().numpy() for s in range(S)])
+        ow, ov = problem.host_weights(seed, S, lo, hi), np.zeros((S, hi - lo), np.float32)
+        for k in range(steps):
+            oracle_mod.step(problem.host_grads(seed, k, S, G, lo, hi, "uniform"), ow, ov, LR, MU, k)
+        assert_parity(gw, gv, ow, ov, True)
+    h.close()
+    torch.cuda.empty_cache()
 
 
 def test_paper_literal_shape(H, oracle_mod):
