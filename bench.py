@@ -51,7 +51,6 @@ def parse_args():
     ap.add_argument("--cpu-sample-elems", type=int, default=1 << 22)
     ap.add_argument("--cpu-sample-steps", type=int, default=20)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
-    ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[4]: bandwidth sweep over P, S, G (one JSON line per point)")
@@ -348,8 +347,8 @@ def run_ours(args):
     S, G, P = cfg["S"], cfg["G"], cfg["P"]
     flags = parse_flags(H, args.flags)
     h = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags, device=local)
-    if args.blocks_per_sm or args.variant:
-        h.hadpsgd_set_launch(args.blocks_per_sm, 0, args.variant)
+    if args.blocks_per_sm:
+        h.hadpsgd_set_launch(args.blocks_per_sm)
     # rank r owns parameters [r*P, (r+1)*P) of an N*P-parameter model: its own seed stream
     seed = 2000 + rank
     problem.fill_weights(h, seed)

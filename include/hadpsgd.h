@@ -157,8 +157,9 @@ int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded);
 /* Synchronises the stream and copies the diagnostics of the most recent step to the host. */
 int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out);
 
-/* Tuning knobs for measurement (persistent grid size, block size, tile order); 0 = default. */
-int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm, int threads_per_block, int variant);
+/* Measurement knob: resident blocks per SM of the persistent grid (1..16, clamped to what fits);
+ * 0 restores the default chosen per (G, dtype, mode).  Results do not depend on it.          */
+int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm);
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int hadpsgd_launch_count(hadpsgd_handle h, uint64_t* out);
 

@@ -69,7 +69,7 @@ def lib():
         L.hadpsgd_segment.argtypes = [vp, i32, i64p, i64p]
         L.hadpsgd_padded_len.argtypes = [vp, i64p]
         L.hadpsgd_diagnostics.argtypes = [vp, ctypes.POINTER(hadpsgd_diag)]
-        L.hadpsgd_set_launch.argtypes = [vp, i32, i32, i32]
+        L.hadpsgd_set_launch.argtypes = [vp, i32]
         L.hadpsgd_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.hadpsgd_error_string.argtypes = [i32]
         L.hadpsgd_error_string.restype = ctypes.c_char_p
@@ -218,8 +218,8 @@ class Hadpsgd:
         _check(lib().hadpsgd_diagnostics(self.h, ctypes.byref(d)), self.h)
         return self._diag_dict(d)
 
-    def hadpsgd_set_launch(self, blocks_per_sm=0, threads=0, variant=0):
-        _check(lib().hadpsgd_set_launch(self.h, blocks_per_sm, threads, variant), self.h)
+    def hadpsgd_set_launch(self, blocks_per_sm=0):
+        _check(lib().hadpsgd_set_launch(self.h, blocks_per_sm), self.h)
 
     def hadpsgd_launch_count(self):
         out = ctypes.c_uint64(0)

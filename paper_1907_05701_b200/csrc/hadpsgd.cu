@@ -30,7 +30,7 @@ struct hadpsgd_ctx {
     uint64_t last_step_k = 0;
     int last_n_pairs = 0;
     uint64_t launches = 0;
-    int blocks_per_sm = 0, threads = 0, variant = 0;   // tuning overrides (0 = default)
+    int blocks_per_sm = 0;   // tuning override of the persistent grid (0 = the plan's default)
     std::string err;
 };
 
@@ -332,9 +332,9 @@ extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
     return HADPSGD_OK;
 }
 
-extern "C" int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm, int threads_per_block, int variant) {
+extern "C" int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm) {
     if (!h || blocks_per_sm < 0 || blocks_per_sm > 16) return HADPSGD_INVALID_ARG;
-    h->blocks_per_sm = blocks_per_sm; h->threads = threads_per_block; h->variant = variant;
+    h->blocks_per_sm = blocks_per_sm;
     return HADPSGD_OK;
 }
 extern "C" int hadpsgd_launch_count(hadpsgd_handle h, uint64_t* out) {
