@@ -33,6 +33,8 @@ def lib():
         L.hadpsgd_oracle_step.argtypes = [i32, i32, i64, vp, i32, vp, vp, f32, f32, u64, u32, vp]
         L.hadpsgd_oracle_step_f64.argtypes = [i32, i32, i64, vp, i32, vp, vp, f64, f64, u64, u32]
         L.hadpsgd_oracle_consensus_distance.argtypes = [i32, i64, vp, vp]
+        L.hadpsgd_oracle_round_bf16.argtypes = [i64, vp, vp]
+        L.hadpsgd_oracle_round_bf16.restype = i32
         for fn in (L.hadpsgd_oracle_partner, L.hadpsgd_oracle_mixing_matrix, L.hadpsgd_oracle_step,
                    L.hadpsgd_oracle_step_f64, L.hadpsgd_oracle_consensus_distance):
             fn.restype = i32
@@ -97,6 +99,16 @@ def step_f64(grads, w, v, lr, mu, step_k, flags=0):
                                        float(lr), float(mu), int(step_k), int(flags))
     if rc != 0:
         raise ValueError(f"hadpsgd_oracle_step_f64 rc={rc}")
+
+
+def round_bf16(w):
+    """bf16 bit patterns (uint16, same shape) of the fp32 array w, round-to-nearest-even."""
+    w = np.ascontiguousarray(w, dtype=np.float32)
+    out = np.empty(w.shape, dtype=np.uint16)
+    rc = lib().hadpsgd_oracle_round_bf16(w.size, _ptr(w), _ptr(out))
+    if rc != 0:
+        raise ValueError("hadpsgd_oracle_round_bf16 failed")
+    return out
 
 
 def consensus_distance(w):

@@ -190,6 +190,43 @@ extern "C" int hadpsgd_oracle_step_f64(int S, int G, int64_t P, const void* grad
     return 0;
 }
 
+extern "C" int hadpsgd_oracle_round_bf16(int64_t n, const float* w, uint16_t* out) {
+    if (n < 0 || !w || !out) return -1;
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t bits;
+        std::memcpy(&bits, &w[i], sizeof bits);
+        const uint32_t expo = (bits >> 23) & 0xFFu;
+        if (expo == 0xFFu) {  // Inf stays Inf; NaN becomes a quiet NaN with the sign kept
+            out[i] = (bits & 0x007FFFFFu) ? static_cast<uint16_t>((bits >> 16) | 0x0040u)
+                                          : static_cast<uint16_t>(bits >> 16);
+            continue;
+        }
+        // the two bf16 neighbours (same sign): magnitude truncated, and one bf16 ulp above it
+        const uint32_t lo_bits = bits & 0xFFFF0000u, hi_bits = lo_bits + 0x00010000u;
+        float lo, hi;
+        std::memcpy(&lo, &lo_bits, sizeof lo);
+        std::memcpy(&hi, &hi_bits, sizeof hi);  // may be +-Inf: overflow rounds there, as IEEE says
+        // distances are exact in double (all three are fp32 values of nearby magnitude); when hi is
+        // Inf the comparison uses the finite value 2^128 that Inf stands in for under IEEE rounding
+        const double x = static_cast<double>(w[i]);
+        const double dlo = x - static_cast<double>(lo);
+        double dhi;
+        if (((hi_bits >> 23) & 0xFFu) == 0xFFu) {
+            const double two128 = 340282366920938463463374607431768211456.0;
+            dhi = ((bits >> 31) ? -two128 : two128) - x;
+        } else {
+            dhi = static_cast<double>(hi) - x;
+        }
+        const double alo = dlo < 0 ? -dlo : dlo, ahi = dhi < 0 ? -dhi : dhi;
+        uint32_t pick;
+        if (alo < ahi) pick = lo_bits;
+        else if (ahi < alo) pick = hi_bits;
+        else pick = ((lo_bits >> 16) & 1u) ? hi_bits : lo_bits;  // tie: even last mantissa bit
+        out[i] = static_cast<uint16_t>(pick >> 16);
+    }
+    return 0;
+}
+
 extern "C" int hadpsgd_oracle_consensus_distance(int S, int64_t P, const float* w, double* out) {
     if (S < 1 || P < 0 || !w || !out) return -1;
     double D = 0.0;

@@ -73,6 +73,14 @@ int hadpsgd_oracle_step_f64(int S, int G, int64_t P,
                             double* w, double* v,
                             double lr, double mu, uint64_t step_k, uint32_t flags);
 
+/* bf16 working copy of fp32 weights for mixed-precision learners (
+ * not in the paper): out[i] = the bf16 value NEAREST to w[i], ties to the value whose last
+ * mantissa bit is even (IEEE round-to-nearest-even to 8 significant bits), written out as the
+ * definition: the two bf16 neighbours of w[i] are compared by exact distance.  NaN -> a quiet
+ * NaN, +-Inf unchanged, overflow past the largest finite bf16 -> +-Inf.  out holds bf16 bit
+ * patterns (uint16).                                                                          */
+int hadpsgd_oracle_round_bf16(int64_t n, const float* w, uint16_t* out);
+
 /* Consensus distance D = sum_s sum_i (w[s][i] - mean_s w[.][i])^2 in double
  * (repeated mixing drives all learners to (1/n) sum theta^i).   */
 int hadpsgd_oracle_consensus_distance(int S, int64_t P, const float* w, double* out);

@@ -404,3 +404,52 @@ def test_invalid_arguments(oracle_mod):
     with pytest.raises(ValueError):
         oracle_mod.step(g, w, v, LR, MU, 0)               # odd S > 1
     oracle_mod.step(g, w, v, LR, MU, 0, flags=oracle_mod.NO_MIX)   # fine without mixing
+
+
+# ------------------------------------------------------------------ bf16 working copy (row f2)
+
+def _all_finite_bf16():
+    bits = np.arange(65536, dtype=np.uint32)
+    vals = (bits << np.uint32(16)).view(np.float32).astype(np.float64)
+    keep = np.isfinite(vals)
+    return bits[keep].astype(np.uint16), vals[keep]
+
+
+def test_round_bf16_brute_force_nearest_ties_to_even(oracle_mod):
+    """Brute force over ALL finite bf16 values: the result must be the nearest one, and on an exact
+    tie the one with an even last mantissa bit (IEEE round-to-nearest-even)."""
+    cand_bits, cand = _all_finite_bf16()
+    rng = np.random.default_rng(5)
+    x = np.concatenate([rand(300, 1, 0.05).ravel(), rand(100, 2, 1e-3).ravel(),
+                        rng.integers(0, 2 ** 32, 400, dtype=np.uint64).astype(np.uint32).view(np.float32)])
+    x = x[np.isfinite(x) & (np.abs(x) < 3.0e38)].astype(np.float32)
+    # exact halfway points between neighbouring bf16 values (fp32 can hold them)
+    ties = ((np.array([0x3F80, 0x3F81, 0x4000, 0x00FF, 0xBF80, 0x3DCC], dtype=np.uint32) << 16) | 0x8000).view(np.float32)
+    x = np.concatenate([x, ties])
+    got = oracle_mod.round_bf16(x)
+    for xi, gi in zip(x.astype(np.float64), got):
+        d = np.abs(cand - xi)
+        best = np.flatnonzero(d == d.min())
+        if (cand[best] == 0).all():                             # +0 / -0 are the same value
+            assert int(gi) in (0x0000, 0x8000)
+        elif len(best) == 1:
+            assert int(gi) == int(cand_bits[best[0]])
+        else:                                                   # tie: even last mantissa bit wins
+            even = [int(b) for b in cand_bits[best] if b % 2 == 0]
+            assert len(even) == 1 and int(gi) == even[0], (xi, hex(int(gi)), [hex(int(b)) for b in cand_bits[best]])
+        assert np.abs(np.float64(gen.bf16_bits_to_f32(np.array([gi], np.uint16))[0]) - xi) == d.min()
+
+
+def test_round_bf16_matches_library_and_fixed_points(oracle_mod):
+    import torch
+    x = rand(200_000, 9, 0.05).ravel()
+    lib = torch.from_numpy(x).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)   # library RNE cast
+    assert np.array_equal(oracle_mod.round_bf16(x), lib)
+    # bf16-representable values are fixed points; widening the result is exact
+    r = gen.bf16_bits_to_f32(oracle_mod.round_bf16(x))
+    assert np.array_equal(oracle_mod.round_bf16(r), oracle_mod.round_bf16(x))
+    assert np.all(np.abs(r.astype(np.float64) - x) <= np.abs(x.astype(np.float64)) * 2.0 ** -8)   # half an ulp of 8 bits
+    sp = np.array([np.inf, -np.inf, 3.4028235e38, -3.4028235e38, 0.0, -0.0], np.float32)
+    assert [int(v) for v in oracle_mod.round_bf16(sp)] == [0x7F80, 0xFF80, 0x7F80, 0xFF80, 0x0000, 0x8000]
+    nan = oracle_mod.round_bf16(np.array([np.nan], np.float32))[0]
+    assert (nan & 0x7F80) == 0x7F80 and (nan & 0x007F) != 0
