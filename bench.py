@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--cpu-sample-steps", type=int, default=20)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7")
+    ap.add_argument("--emit-bf16", action="store_true",
+                    help="also write the bf16 working copy of the weights every step (row f2; +2 B/param)")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[4]: bandwidth sweep over P, S, G (one JSON line per point)")
     ap.add_argument("--sweep-md", default="", help="also write the sweep as a markdown table to this path")
@@ -67,8 +69,9 @@ def workload(name):
 
 
 def algorithmic_bytes(cfg):
-    """per parameter per super-learner, read G*b_g + 4 (w) + 4 (v), write 4 + 4."""
-    return cfg["S"] * cfg["P"] * (cfg["G"] * cfg["b_g"] + 16)
+    """per parameter per super-learner, read G*b_g + 4 (w) + 4 (v), write 4 + 4
+    (+ 2 when the bf16 working copy is emitted)."""
+    return cfg["S"] * cfg["P"] * (cfg["G"] * cfg["b_g"] + 16 + (2 if cfg.get("emit") else 0))
 
 
 def measured_peak():
@@ -344,9 +347,11 @@ def run_ours(args):
     assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world} (launch N>1 with torch.distributed.run)"
 
     cfg = workload(args.workload)
+    cfg["emit"] = args.emit_bf16
     S, G, P = cfg["S"], cfg["G"], cfg["P"]
     flags = parse_flags(H, args.flags)
-    h = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags, device=local)
+    h = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags, device=local,
+                  working_dtype=H.BF16 if args.emit_bf16 else H.F32)
     if args.blocks_per_sm:
         h.hadpsgd_set_launch(args.blocks_per_sm)
     # rank r owns parameters [r*P, (r+1)*P) of an N*P-parameter model: its own seed stream
@@ -387,12 +392,14 @@ def run_ours(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "S": S, "G": G, "P": P, "n_segments": len(cfg["seg_len"]),
-                       "grad_dtype": cfg["grad"], "master_dtype": "f32", "lr": LR, "momentum": MU,
+                       "grad_dtype": cfg["grad"], "master_dtype": "f32",
+                       "working_dtype": "bf16" if args.emit_bf16 else "f32", "lr": LR, "momentum": MU,
                        "resident_bytes_per_gpu": h.arena_bytes, "flags": args.flags or "default (diagnostics on)",
                        "l2": "inputs larger than L2 (working set per step >> 126 MB); no flush needed",
                        "parallelism": "single GPU" if world == 1 else f"parameter-range shards x{world}, no data-path collective"},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(args.workload), "traffic_source": NCU_TRAFFIC_SOURCE.get(args.workload),
+                         "traffic": None if args.emit_bf16 else NCU_TRAFFIC_BYTES.get(args.workload),
+                         "traffic_source": None if args.emit_bf16 else NCU_TRAFFIC_SOURCE.get(args.workload),
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
                          "kernel": "hadpsgd::step_kernel (one launch = one step)", "frac_of_8TBps_nominal": achieved / 8000.0},
             "clocks": clocks, "gpu_launches": launches,

@@ -65,6 +65,10 @@ enum { /* hadpsgd_opts.flags */
 typedef struct {
     int32_t grad_dtype;   /* HADPSGD_F32 | HADPSGD_BF16 : dtype of the S*G learner gradient buffers */
     int32_t master_dtype; /* must be HADPSGD_F32 : weights AND momentum                             */
+    int32_t working_dtype;/* HADPSGD_F32 (0, default): learners read the fp32 master weights, nothing
+                             extra is stored.  HADPSGD_BF16: every step ALSO writes a bf16
+                             (round-to-nearest-even) copy of each new weight buffer for
+                             mixed-precision learners (+2 B per parameter per super-learner; row f2) */
 } hadpsgd_dtypes;
 
 typedef struct {
@@ -95,10 +99,11 @@ int hadpsgd_required_bytes(int S, int G, const int64_t* seg_len /*host [n_seg]*/
  * the weight, momentum and gradient regions inside the arena (each may be NULL).
  * weight buffer s   = arena + w_off + s * P_padded * 4
  * momentum buffer s = arena + v_off + s * P_padded * 4
- * gradient (s,g)    = arena + g_off + (s*G + g) * P_padded * sizeof(grad_dtype)               */
+ * gradient (s,g)    = arena + g_off + (s*G + g) * P_padded * sizeof(grad_dtype)
+ * bf16 working copy s = arena + wb_off + s * P_padded * 2   (only with working_dtype == BF16)  */
 int hadpsgd_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
                    int64_t* seg_offset, int64_t* P_padded,
-                   size_t* w_off, size_t* v_off, size_t* g_off);
+                   size_t* w_off, size_t* v_off, size_t* g_off, size_t* wb_off);
 
 /* a1 pairing scheduler (pure host function) -------------------------------------------------- */
 
@@ -151,6 +156,9 @@ int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads /*host [S*
 int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr);
 int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr);
 int hadpsgd_grads(hadpsgd_handle h, int s, int g, void** dev_ptr);
+/* bf16 working copy of super-learner s's weights (P_padded bf16 values, rewritten by every step;
+ * zero until the first step).  INVALID_ARG unless created with working_dtype == HADPSGD_BF16. */
+int hadpsgd_weights_bf16(hadpsgd_handle h, int s, void** dev_ptr);
 int hadpsgd_segment(hadpsgd_handle h, int seg, int64_t* elem_offset, int64_t* elem_len);
 int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded);
 

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libhadpsgd.so")
 
 
 class hadpsgd_dtypes(ctypes.Structure):
-    _fields_ = [("grad_dtype", ctypes.c_int32), ("master_dtype", ctypes.c_int32)]
+    _fields_ = [("grad_dtype", ctypes.c_int32), ("master_dtype", ctypes.c_int32), ("working_dtype", ctypes.c_int32)]
 
 
 class hadpsgd_opts(ctypes.Structure):
@@ -53,7 +53,7 @@ def lib():
         i32, i64p, vp, sz_p = ctypes.c_int, ctypes.POINTER(ctypes.c_int64), ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t)
         f32, u64 = ctypes.c_float, ctypes.c_uint64
         L.hadpsgd_required_bytes.argtypes = [i32, i32, i64p, i32, hadpsgd_dtypes, sz_p]
-        L.hadpsgd_layout.argtypes = [i32, i32, i64p, i32, hadpsgd_dtypes, i64p, i64p, sz_p, sz_p, sz_p]
+        L.hadpsgd_layout.argtypes = [i32, i32, i64p, i32, hadpsgd_dtypes, i64p, i64p, sz_p, sz_p, sz_p, sz_p]
         L.hadpsgd_pairing.argtypes = [i32, u64, ctypes.POINTER(ctypes.c_int32)]
         L.hadpsgd_shard_range.argtypes = [ctypes.c_int64, i32, i32, i64p, i64p]
         L.hadpsgd_lr_schedule.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double, i32, i32,
@@ -66,6 +66,7 @@ def lib():
         L.hadpsgd_weights.argtypes = [vp, i32, ctypes.POINTER(vp)]
         L.hadpsgd_momentum.argtypes = [vp, i32, ctypes.POINTER(vp)]
         L.hadpsgd_grads.argtypes = [vp, i32, i32, ctypes.POINTER(vp)]
+        L.hadpsgd_weights_bf16.argtypes = [vp, i32, ctypes.POINTER(vp)]
         L.hadpsgd_segment.argtypes = [vp, i32, i64p, i64p]
         L.hadpsgd_padded_len.argtypes = [vp, i64p]
         L.hadpsgd_diagnostics.argtypes = [vp, ctypes.POINTER(hadpsgd_diag)]
@@ -91,21 +92,22 @@ def _check(rc, h=None):
         raise HadpsgdError(rc, f"{L.hadpsgd_error_string(rc).decode()}: {detail}")
 
 
-def hadpsgd_required_bytes(S, G, seg_len, grad_dtype=F32):
+def hadpsgd_required_bytes(S, G, seg_len, grad_dtype=F32, working_dtype=F32):
     arr, n = _seg(seg_len)
     out = ctypes.c_size_t(0)
-    _check(lib().hadpsgd_required_bytes(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32), ctypes.byref(out)))
+    _check(lib().hadpsgd_required_bytes(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype), ctypes.byref(out)))
     return out.value
 
 
-def hadpsgd_layout(S, G, seg_len, grad_dtype=F32):
+def hadpsgd_layout(S, G, seg_len, grad_dtype=F32, working_dtype=F32):
     arr, n = _seg(seg_len)
     seg_off = (ctypes.c_int64 * n)()
     P = ctypes.c_int64(0)
-    w, v, g = ctypes.c_size_t(0), ctypes.c_size_t(0), ctypes.c_size_t(0)
-    _check(lib().hadpsgd_layout(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32), seg_off, ctypes.byref(P),
-                                ctypes.byref(w), ctypes.byref(v), ctypes.byref(g)))
-    return dict(seg_offset=list(seg_off), P_padded=P.value, w_off=w.value, v_off=v.value, g_off=g.value)
+    w, v, g, wb = ctypes.c_size_t(0), ctypes.c_size_t(0), ctypes.c_size_t(0), ctypes.c_size_t(0)
+    _check(lib().hadpsgd_layout(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype), seg_off, ctypes.byref(P),
+                                ctypes.byref(w), ctypes.byref(v), ctypes.byref(g), ctypes.byref(wb)))
+    return dict(seg_offset=list(seg_off), P_padded=P.value, w_off=w.value, v_off=v.value, g_off=g.value,
+                wb_off=wb.value)
 
 
 def hadpsgd_pairing(S, step_k):
@@ -130,17 +132,18 @@ class Hadpsgd:
     """Handle wrapper.  Device memory is a torch uint8 tensor (the arena) so that torch owns
     allocation and stream plumbing; everything else happens behind the C ABI."""
 
-    def __init__(self, S, G, seg_len, grad_dtype=F32, flags=0, device=0, stream=None, own_arena=False):
+    def __init__(self, S, G, seg_len, grad_dtype=F32, flags=0, device=0, stream=None, own_arena=False,
+                 working_dtype=F32):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("hadpsgd needs a CUDA device (sm_100a); there is no CPU fallback")
         self.S, self.G, self.seg_len = int(S), int(G), [int(x) for x in seg_len]
-        self.grad_dtype, self.flags = grad_dtype, flags
+        self.grad_dtype, self.flags, self.working_dtype = grad_dtype, flags, working_dtype
         self.torch = torch
         self.device = torch.device("cuda", device)
         arr, n = _seg(self.seg_len)
-        nbytes = hadpsgd_required_bytes(S, G, self.seg_len, grad_dtype)
-        self.layout = hadpsgd_layout(S, G, self.seg_len, grad_dtype)
+        nbytes = hadpsgd_required_bytes(S, G, self.seg_len, grad_dtype, working_dtype)
+        self.layout = hadpsgd_layout(S, G, self.seg_len, grad_dtype, working_dtype)
         self.P_padded = self.layout["P_padded"]
         opts = hadpsgd_opts()
         opts.flags, opts.device = flags, device
@@ -155,7 +158,8 @@ class Hadpsgd:
         self.arena_bytes = nbytes
         h = ctypes.c_void_p()
         with torch.cuda.device(self.device):
-            _check(lib().hadpsgd_create(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32), ctypes.byref(opts), ctypes.byref(h)))
+            _check(lib().hadpsgd_create(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype), ctypes.byref(opts),
+                                        ctypes.byref(h)))
         self.h = h
 
     # -- the three core calls ------------------------------------------------------------
@@ -197,6 +201,11 @@ class Hadpsgd:
         _check(lib().hadpsgd_grads(self.h, s, g, ctypes.byref(p)), self.h)
         dt = self.torch.bfloat16 if self.grad_dtype == BF16 else self.torch.float32
         return self._view(p.value, self.P_padded, dt)
+
+    def hadpsgd_weights_bf16(self, s):
+        p = ctypes.c_void_p()
+        _check(lib().hadpsgd_weights_bf16(self.h, s, ctypes.byref(p)), self.h)
+        return self._view(p.value, self.P_padded, self.torch.bfloat16)
 
     def hadpsgd_grads_ptr(self, s, g):
         p = ctypes.c_void_p()

@@ -6,11 +6,13 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhadpsgd.so")
-SOURCES = ["hadpsgd.cu", "allocator.cpp", "scheduler.cpp", "schedule.cpp"]
-DEPS = SOURCES + ["internal.h", "step_kernel.cuh", os.path.join("..", "..", "include", "hadpsgd.h")]
+SOURCES = ["hadpsgd.cu", "step_f32.cu", "step_bf16.cu", "step_f32_emit.cu", "step_bf16_emit.cu",
+           "allocator.cpp", "scheduler.cpp", "schedule.cpp"]
+DEPS = SOURCES + ["internal.h", "step_kernel.cuh", "step_dispatch.cuh", os.path.join("..", "..", "include", "hadpsgd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--ftz=false", "--prec-div=true", "--prec-sqrt=true",   # IEEE: no flush-to-zero (R17)
-              "-Xcompiler", "-fPIC,-Wall", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC,-Wall", "-shared", "-cudart", "static",
+              "--threads", "4"]           # the four step_*.cu instantiation units compile in parallel
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -5,7 +5,8 @@
 // aligned to HADPSGD_SEG_ALIGN_ELEMS elements in every buffer (
 // north_star (a)).  One weight + one momentum copy per SUPER-learner: the G learners of a
 // super-learner have staleness 0, so their replicas are identical and are
-// collapsed (R18).
+// collapsed (R18).  With dtypes.working_dtype == BF16 a fourth region holds S bf16
+// working copies of the weights (row f2).
 #include "internal.h"
 
 namespace hadpsgd {
@@ -21,9 +22,10 @@ int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
     if (n_seg < 1 || !seg_len) return fail("segment table must have at least one segment");
     if (dt.grad_dtype != HADPSGD_F32 && dt.grad_dtype != HADPSGD_BF16) return fail("grad_dtype must be F32 or BF16");
     if (dt.master_dtype != HADPSGD_F32) return fail("master_dtype must be F32");
+    if (dt.working_dtype != HADPSGD_F32 && dt.working_dtype != HADPSGD_BF16) return fail("working_dtype must be F32 (none) or BF16");
 
     Layout L;
-    L.S = S; L.G = G; L.n_seg = n_seg; L.grad_dtype = dt.grad_dtype;
+    L.S = S; L.G = G; L.n_seg = n_seg; L.grad_dtype = dt.grad_dtype; L.working_dtype = dt.working_dtype;
     L.seg_len.assign(seg_len, seg_len + n_seg);
     L.seg_offset.resize(n_seg);
     int64_t off = 0;
@@ -41,6 +43,8 @@ int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
     L.w_off = cur; cur = round_up(cur + static_cast<size_t>(S) * L.w_stride_bytes(), kRegionAlign);
     L.v_off = cur; cur = round_up(cur + static_cast<size_t>(S) * L.w_stride_bytes(), kRegionAlign);
     L.g_off = cur; cur = round_up(cur + static_cast<size_t>(S) * G * L.g_stride_bytes(), kRegionAlign);
+    L.wb_off = cur;
+    if (L.working_dtype == HADPSGD_BF16) cur = round_up(cur + static_cast<size_t>(S) * L.P_padded * 2, kRegionAlign);
     // aux: per-block partial sums [S items][5][kMaxGridBlocks] doubles, results [3*S] doubles, ticket
     L.aux_off = cur;
     L.aux_bytes = round_up(static_cast<size_t>(S) * kDiagQuantities * kMaxGridBlocks * sizeof(double) +
@@ -65,7 +69,7 @@ extern "C" int hadpsgd_required_bytes(int S, int G, const int64_t* seg_len, int 
 
 extern "C" int hadpsgd_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
                               int64_t* seg_offset, int64_t* P_padded, size_t* w_off, size_t* v_off,
-                              size_t* g_off) {
+                              size_t* g_off, size_t* wb_off) {
     hadpsgd::Layout L;
     int rc = hadpsgd::compute_layout(S, G, seg_len, n_seg, dt, &L, nullptr);
     if (rc != HADPSGD_OK) return rc;
@@ -74,5 +78,6 @@ extern "C" int hadpsgd_layout(int S, int G, const int64_t* seg_len, int n_seg, h
     if (w_off) *w_off = L.w_off;
     if (v_off) *v_off = L.v_off;
     if (g_off) *g_off = L.g_off;
+    if (wb_off) *wb_off = L.wb_off;
     return HADPSGD_OK;
 }

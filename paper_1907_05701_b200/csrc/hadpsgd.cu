@@ -9,7 +9,7 @@
 #include <vector>
 
 #include "internal.h"
-#include "step_kernel.cuh"
+#include "step_dispatch.cuh"
 
 using namespace hadpsgd;
 
@@ -48,63 +48,22 @@ static thread_local std::string g_create_error;
 // ---- kernel dispatch -------------------------------------------------------------------
 namespace {
 
-struct LaunchPlan { const void* fn; int threads; int tile_units; int blocks_per_sm; };
-
-// Launch shape: 256 threads, ONE resident block per SM, and
-// enough 32-byte loads per thread (>= 12) that ~96 KB per SM are in flight.  More resident
-// warps than that measured slower on this path (more DRAM pages open at once).
-template <int G, bool BF16, bool EXACT, bool DIAG, int MODE>
-LaunchPlan plan_for() {
-    constexpr int members = (MODE == kSingle) ? 1 : 2;
-    constexpr int loads_per_unit = members * ((G > 0 ? G : 4) + (BF16 ? 4 : 2));
-    constexpr int U = loads_per_unit <= 6 ? 2 : 1;
-    // measured: 12 loads x 256 threads and 20 loads x 160 threads
-    // (both ~100 KB in flight per SM) are the best shapes for fp32 G=4 and G=8; 8 loads x 256
-    // threads x 1 block beats both 2 blocks/SM and U=2 for G=2.
-    constexpr int THREADS = (!BF16 && G > 0 && U * loads_per_unit >= 20) ? 160 : 256;
-    constexpr int in_flight = THREADS * U * loads_per_unit * 32;           // bytes per block
-    constexpr int BPS = in_flight >= 48 * 1024 ? 1 : 2;
-    return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, U, THREADS, 1>), THREADS,
-            THREADS * U, BPS};
-}
-
-template <int G, bool BF16, bool EXACT, bool DIAG>
-LaunchPlan pick_mode(int mode) {
-    switch (mode) {
-        case kPair: return plan_for<G, BF16, EXACT, DIAG, kPair>();
-        case kSingle: return plan_for<G, BF16, EXACT, DIAG, kSingle>();
-        default: return plan_for<G, BF16, EXACT, DIAG, kPairEq7>();
-    }
-}
-template <int G, bool BF16>
-LaunchPlan pick_flags(bool exact, bool diag, int mode) {
-    if (exact) return diag ? pick_mode<G, BF16, true, true>(mode) : pick_mode<G, BF16, true, false>(mode);
-    return diag ? pick_mode<G, BF16, false, true>(mode) : pick_mode<G, BF16, false, false>(mode);
-}
-template <bool BF16>
-LaunchPlan pick_G(int G, bool exact, bool diag, int mode) {
-    switch (G) {
-        case 1: return pick_flags<1, BF16>(exact, diag, mode);
-        case 2: return pick_flags<2, BF16>(exact, diag, mode);
-        case 4: return pick_flags<4, BF16>(exact, diag, mode);
-        case 8: return pick_flags<8, BF16>(exact, diag, mode);
-        default: return pick_flags<0, BF16>(exact, diag, mode);  // runtime learner count
-    }
-}
-
 int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     if (items.empty() || elem_end <= elem_begin) return HADPSGD_OK;
     const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
     const bool exact = h->flags & HADPSGD_DETERMINISTIC;
     const bool diag = !(h->flags & HADPSGD_NO_DIAG);
-    LaunchPlan plan = bf16 ? pick_G<true>(h->L.G, exact, diag, mode) : pick_G<false>(h->L.G, exact, diag, mode);
+    const bool emit = h->L.working_dtype == HADPSGD_BF16;
+    LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode) : plan_f32_emit(h->L.G, exact, diag, mode))
+                           : (bf16 ? plan_bf16(h->L.G, exact, diag, mode) : plan_f32(h->L.G, exact, diag, mode));
 
     const int unit = bf16 ? 16 : 8;   // elements per 32-byte gradient vector
     StepArgs a;
     a.w = reinterpret_cast<float*>(h->arena + h->L.w_off);
     a.v = reinterpret_cast<float*>(h->arena + h->L.v_off);
     a.g = h->arena + h->L.g_off;
+    a.wb = emit ? h->arena + h->L.wb_off : nullptr;
     a.P = h->L.P_padded;
     a.unit_begin = elem_begin / unit;
     a.unit_end = elem_end / unit;
@@ -299,6 +258,12 @@ extern "C" int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr) {
 extern "C" int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr) {
     if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
     *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.v_off + static_cast<size_t>(s) * h->L.w_stride_bytes());
+    return HADPSGD_OK;
+}
+extern "C" int hadpsgd_weights_bf16(hadpsgd_handle h, int s, void** dev_ptr) {
+    if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
+    if (h->L.working_dtype != HADPSGD_BF16) { h->err = "handle was created without a bf16 working copy (dtypes.working_dtype)"; return HADPSGD_INVALID_ARG; }
+    *dev_ptr = h->arena + h->L.wb_off + static_cast<size_t>(s) * static_cast<size_t>(h->L.P_padded) * 2;
     return HADPSGD_OK;
 }
 extern "C" int hadpsgd_grads(hadpsgd_handle h, int s, int g, void** dev_ptr) {

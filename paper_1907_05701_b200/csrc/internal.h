@@ -17,9 +17,11 @@ constexpr size_t kRegionAlign = 256;  // byte alignment of every buffer start in
 struct Layout {
     int S = 0, G = 0, n_seg = 0;
     int grad_dtype = HADPSGD_F32;
+    int working_dtype = HADPSGD_F32;         // HADPSGD_BF16: a bf16 copy of the weights is emitted
     int64_t P_padded = 0;
     std::vector<int64_t> seg_len, seg_offset;
     size_t w_off = 0, v_off = 0, g_off = 0;  // byte offsets inside the arena
+    size_t wb_off = 0;                       // bf16 working copies (S x P_padded x 2 B), if any
     size_t aux_off = 0, aux_bytes = 0;       // diagnostics scratch (partials, results, ticket)
     size_t total_bytes = 0;
     size_t grad_elem_bytes() const { return grad_dtype == HADPSGD_BF16 ? 2 : 4; }

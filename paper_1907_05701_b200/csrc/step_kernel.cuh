@@ -8,7 +8,8 @@
 //   * reduces the G gradients left to right in fp32 registers (eq. (6))
 //   * v <- mu v + gbar ; u = w - lr v                       (eq. (3), + momentum)
 //   * w_s = w_p = 1/2 (u_s + u_p)                           (eq. (7))
-//   * writes v_s, v_p, w_s, w_p (32 B stores), and accumulates the a5 diagnostics.
+//   * writes v_s, v_p, w_s, w_p (32 B stores), optionally a bf16 copy of w' (EMIT), and
+//     accumulates the a5 diagnostics.
 // The path is HBM-bound (0.3 flop/B): no tensor cores, no shared-memory staging of data --
 // each byte is touched exactly once, so the design goal is only "the right amount of coalesced
 // 32 B requests in flight per SM" (~100 KB) and full-sector writes.
@@ -32,6 +33,7 @@ struct StepArgs {
     float* w;             // S buffers of P floats
     float* v;             // S buffers of P floats
     const void* g;        // S*G buffers of P grad elements
+    void* wb;             // EMIT only: S buffers of P bf16, the working copy of the new weights
     long long P;          // padded elements per buffer
     long long unit_begin; // first vector unit of this launch
     long long unit_end;   // one past the last vector unit
@@ -125,6 +127,28 @@ __device__ __forceinline__ void store_state(float* base, long long off, const Ve
     }
 }
 
+// EMIT: bf16 (round-to-nearest-even) copy of the new weights for mixed-precision learners
+// (SURVEY.md 8(f) row f2).  8 floats -> one 16 B store, 16 floats -> one 32 B store.
+template <int UNIT>
+__device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<UNIT>& in) {
+    unsigned pk[UNIT / 2];
+#pragma unroll
+    for (int q = 0; q < UNIT / 2; ++q) {
+        __nv_bfloat162 h = __floats2bfloat162_rn(in.x[2 * q], in.x[2 * q + 1]);   // .x = low half
+        pk[q] = *reinterpret_cast<unsigned*>(&h);
+    }
+    __nv_bfloat16* dst = static_cast<__nv_bfloat16*>(base) + off;
+    if constexpr (UNIT == 16) {
+        Raw8 r;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) r.u[q] = pk[q];
+        st_stream32(dst, r);
+    } else {
+        // 16 B streaming store (an L2 evict-first cache-hint policy measured the same)
+        __stcs(reinterpret_cast<uint4*>(dst), make_uint4(pk[0], pk[1], pk[2], pk[3]));
+    }
+}
+
 // Sum of the G learner gradients of one unit, left to right (a2); gradients already in registers.
 template <int G, bool BF16, bool EXACT, int UNIT>
 __device__ __forceinline__ void sum_grads(const Raw8 (&gr)[G], Vec<UNIT>& acc) {
@@ -204,7 +228,7 @@ __device__ __forceinline__ double warp_sum(double x) {
 // THREADS x U units; thread t owns units t, t+THREADS, ... of the tile, so each warp request
 // covers 1 KB contiguous of one stream.
 // ---------------------------------------------------------------------------------------
-template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, int U, int THREADS, int MINB>
+template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, bool EMIT, int U, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_constant__ StepArgs a) {
     constexpr int UNIT = BF16 ? 16 : 8;
     constexpr int GA = G > 0 ? G : 1;
@@ -343,9 +367,11 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 
                 store_state<UNIT>(a.v, os, vs[q]);
                 store_state<UNIT>(a.w, os, outs);
+                if constexpr (EMIT) store_bf16<UNIT>(a.wb, os, outs);
                 if constexpr (PAIRED) {
                     store_state<UNIT>(a.v, op, vp[q]);
                     store_state<UNIT>(a.w, op, MODE == kPair ? outs : outp);
+                    if constexpr (EMIT) store_bf16<UNIT>(a.wb, op, MODE == kPair ? outs : outp);
                 }
 
                 if constexpr (DIAG) {

@@ -75,6 +75,15 @@ def test_allocator_layout(H):
     assert lay["P_padded"] == 192 + 1088 + 128 + 128
     for off in ("w_off", "v_off", "g_off"):
         assert lay[off] % 256 == 0
+    # bf16 working copy (row f2): a fourth region of S x P_padded x 2 B after the gradients
+    plain, emit = H.hadpsgd_layout(4, 2, odd), H.hadpsgd_layout(4, 2, odd, H.F32, H.BF16)
+    assert {k: emit[k] for k in ("seg_offset", "P_padded", "w_off", "v_off", "g_off")} == \
+           {k: plain[k] for k in ("seg_offset", "P_padded", "w_off", "v_off", "g_off")}
+    assert emit["wb_off"] % 256 == 0 and emit["wb_off"] >= emit["g_off"] + 4 * 2 * emit["P_padded"] * 4
+    extra = H.hadpsgd_required_bytes(4, 2, odd, H.F32, H.BF16) - H.hadpsgd_required_bytes(4, 2, odd)
+    assert 4 * emit["P_padded"] * 2 <= extra < 4 * emit["P_padded"] * 2 + 256
+    with pytest.raises(H.HadpsgdError):
+        H.hadpsgd_required_bytes(4, 2, odd, H.F32, 7)
     for bad in ((0, 1, [4]), (2, 0, [4]), (2, 2, []), (2, 2, [4, 0]), (513 * 2, 1, [4])):
         with pytest.raises(H.HadpsgdError):
             H.hadpsgd_required_bytes(*bad)

@@ -298,6 +298,47 @@ def test_error_codes(H, torch_cuda):
     assert rc == b.OUT_OF_MEMORY and not hh
 
 
+@pytest.mark.parametrize("bf16_grads,S,G,flagname", [(False, 4, 4, None), (True, 4, 8, None), (False, 2, 3, None),
+                                                     (True, 3, 2, "NO_MIX"), (False, 4, 2, "EQ7_LITERAL")])
+def test_bf16_working_copy(H, oracle_mod, torch_cuda, bf16_grads, S, G, flagname):
+    """dtypes.working_dtype = BF16 (row f2): every step also writes bf16(w') round-to-nearest-even.
+    Deterministic mode: the copy equals the oracle's rounding of the oracle's weights, bit for bit;
+    default mode: it is the correct rounding of the weights the GPU itself produced.  Ragged table,
+    so the copy's padding must stay zero too."""
+    torch = torch_cuda
+    from fixtures import problem
+    seg, seed, steps = ODD_TABLE, 111, 3
+    P = sum(seg)
+    extra = getattr(H, flagname) if flagname else 0
+    oflags = getattr(oracle_mod, flagname) if flagname in ("NO_MIX", "EQ7_LITERAL") else 0
+    for exact in (True, False):
+        h = H.Hadpsgd(S, G, seg, H.BF16 if bf16_grads else H.F32, (H.DETERMINISTIC if exact else 0) | extra,
+                      working_dtype=H.BF16)
+        problem.fill_weights(h, seed)
+        ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+        assert not h.hadpsgd_weights_bf16(0).view(torch.int16).any()          # zero until the first step
+        for k in range(steps):
+            problem.fill_grads(h, seed, k)
+            h.hadpsgd_step(LR, MU, k)
+            oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P, bf16=bf16_grads), ow, ov, LR, MU, k, flags=oflags)
+        torch.cuda.synchronize()
+        nat = torch.from_numpy(h.natural_index()).cuda()
+        gw = np.stack([h.hadpsgd_weights(s)[nat].cpu().numpy() for s in range(S)])
+        gb = np.stack([h.hadpsgd_weights_bf16(s).view(torch.int16)[nat].cpu().numpy().view(np.uint16) for s in range(S)])
+        assert np.array_equal(gb, oracle_mod.round_bf16(gw))                  # correct rounding of the GPU's own w'
+        if exact:
+            assert np.array_equal(bits(gw), bits(ow))
+            assert np.array_equal(gb, oracle_mod.round_bf16(ow))
+        mask = torch.ones(h.P_padded, dtype=torch.bool, device="cuda"); mask[nat] = False
+        for s in range(S):
+            assert not h.hadpsgd_weights_bf16(s).view(torch.int16)[mask].any()
+        h.close()
+    plain = H.Hadpsgd(2, 2, [100])
+    with pytest.raises(H.HadpsgdError):
+        plain.hadpsgd_weights_bf16(0)
+    plain.close()
+
+
 def test_cuda_graph_capture_and_replay(H, oracle_mod, torch_cuda):
     """hadpsgd_step only enqueues on its stream, so an (even, odd) step pair can be captured into a
     CUDA graph and replayed; 3 replays = 6 steps must equal 6 oracle steps bit for bit."""
