@@ -44,8 +44,9 @@ enum { HADPSGD_F32 = 0, HADPSGD_BF16 = 1 };
 
 enum { /* status codes */
     HADPSGD_OK = 0,
-    HADPSGD_INVALID_ARG = -1,        /* S<1, S odd and >1 (unless NO_MIX), G<1, n_seg<1, seg_len<1,
-                                        bad dtype, index out of range, NULL out-pointer, S>HADPSGD_MAX_S */
+    HADPSGD_INVALID_ARG = -1,        /* S<1, S>HADPSGD_MAX_S, G<1, n_seg<1, seg_len<1, bad dtype, index out
+                                        of range, NULL out-pointer, a partner[] that is not a matching;
+                                        hadpsgd_step with S odd and >1 (no perfect ring matching)      */
     HADPSGD_OUT_OF_MEMORY = -2,      /* arena too small / cudaMalloc failed                                */
     HADPSGD_CUDA = -3,               /* CUDA runtime or launch error; text via hadpsgd_last_error()        */
     HADPSGD_UNSUPPORTED_DEVICE = -4  /* compute capability != 10.x: no multi-backend dispatch, no fallback */
@@ -136,6 +137,8 @@ int hadpsgd_destroy(hadpsgd_handle h);
 /* a2-a6 the step ----------------------------------------------------------------------------- */
 
 /* Enqueue one fused step (one kernel launch) on the handle's stream; asynchronous.
+ * S odd and > 1 admits no perfect ring matching (R8): INVALID_ARG unless the handle
+ * was created with HADPSGD_NO_MIX -- use hadpsgd_step_matching with an unpaired member instead.
  * Gradient buffers are read-only to the step (not zeroed); w and v are updated in place.
  * step_k is used only for its parity (no hidden counter: a step can be replayed).           */
 int hadpsgd_step(hadpsgd_handle h, float lr, float momentum, uint64_t step_k);
@@ -164,6 +167,12 @@ int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded);
 
 /* Synchronises the stream and copies the diagnostics of the most recent step to the host. */
 int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out);
+
+/* Consensus distance D = sum_i sum_s (w_s[i] - mean_s w_.[i])^2 of the current weights
+ * (mixing alone drives every learner to the mean; D measures how far they are).
+ * Optional, NOT part of the step: one extra kernel that reads the S weight buffers once, then
+ * synchronises the stream.  D_out: host.  Identity: D(u) - D(w') = 1/2 sum_pairs gap.         */
+int hadpsgd_consensus(hadpsgd_handle h, double* D_out);
 
 /* Measurement knob: resident blocks per SM of the persistent grid (1..16, clamped to what fits);
  * 0 restores the default chosen per (G, dtype, mode).  Results do not depend on it.          */

@@ -70,6 +70,7 @@ def lib():
         L.hadpsgd_segment.argtypes = [vp, i32, i64p, i64p]
         L.hadpsgd_padded_len.argtypes = [vp, i64p]
         L.hadpsgd_diagnostics.argtypes = [vp, ctypes.POINTER(hadpsgd_diag)]
+        L.hadpsgd_consensus.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
         L.hadpsgd_set_launch.argtypes = [vp, i32]
         L.hadpsgd_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.hadpsgd_error_string.argtypes = [i32]
@@ -226,6 +227,11 @@ class Hadpsgd:
         d = hadpsgd_diag()
         _check(lib().hadpsgd_diagnostics(self.h, ctypes.byref(d)), self.h)
         return self._diag_dict(d)
+
+    def hadpsgd_consensus(self):
+        out = ctypes.c_double(0.0)
+        _check(lib().hadpsgd_consensus(self.h, ctypes.byref(out)), self.h)
+        return out.value
 
     def hadpsgd_set_launch(self, blocks_per_sm=0):
         _check(lib().hadpsgd_set_launch(self.h, blocks_per_sm), self.h)

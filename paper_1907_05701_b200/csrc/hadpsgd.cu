@@ -120,7 +120,8 @@ int build_partner(hadpsgd_ctx* h, uint64_t step_k, const int32_t* custom, std::v
     } else if (h->flags & HADPSGD_NO_MIX) {
         for (int s = 0; s < S; ++s) (*partner)[s] = s;
     } else if (ring_partner(S, step_k, partner->data()) != HADPSGD_OK) {
-        h->err = "no perfect ring matching for odd S > 1";
+        h->err = "odd S > 1 has no perfect ring matching (PAPER.md:66 needs two 0.5s per row): use "
+                 "hadpsgd_step_matching with an unpaired member (T_ii = 1) or HADPSGD_NO_MIX";
         return HADPSGD_INVALID_ARG;
     }
     return HADPSGD_OK;
@@ -139,11 +140,6 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
     int rc = compute_layout(S, G, seg_len, n_seg, dt, &L, &why);
     if (rc != HADPSGD_OK) { g_create_error = why; return rc; }
     const uint32_t flags = opts ? opts->flags : 0u;
-    if (S > 1 && (S & 1) && !(flags & HADPSGD_NO_MIX)) {
-        g_create_error = "odd S > 1 has no perfect ring matching (PAPER.md:66 needs two 0.5s per row; use HADPSGD_NO_MIX for unmixed runs)";
-        return HADPSGD_INVALID_ARG;
-    }
-
     int dev = (opts && opts->device >= 0) ? opts->device : -1;
     cudaError_t e;
     if (dev < 0) { e = cudaGetDevice(&dev); } else { e = cudaSetDevice(dev); }
@@ -294,6 +290,28 @@ extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
     std::memcpy(host_out->gsq, tmp.data(), sizeof(double) * S);
     std::memcpy(host_out->wsq, tmp.data() + S, sizeof(double) * S);
     std::memcpy(host_out->gap, tmp.data() + 2 * S, sizeof(double) * S);
+    return HADPSGD_OK;
+}
+
+namespace hadpsgd {
+int launch_consensus(const float* w, long long P_padded, int S, int num_sms, double* block_out,
+                     cudaStream_t stream, cudaError_t* err);   // consensus.cu
+}
+
+extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
+    if (!h || !D_out) return HADPSGD_INVALID_ARG;
+    // the partials scratch is free between steps: everything is ordered on h->stream
+    cudaError_t e = cudaSuccess;
+    const int grid = launch_consensus(reinterpret_cast<const float*>(h->arena + h->L.w_off), h->L.P_padded, h->L.S,
+                                      h->num_sms, h->d_partials, h->stream, &e);
+    CUDA_TRY(h, e);
+    h->launches++;
+    std::vector<double> part(grid);
+    CUDA_TRY(h, cudaMemcpyAsync(part.data(), h->d_partials, sizeof(double) * grid, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    double D = 0.;
+    for (int b = 0; b < grid; ++b) D += part[b];   // fixed order: run-to-run deterministic
+    *D_out = D;
     return HADPSGD_OK;
 }
 

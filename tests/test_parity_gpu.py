@@ -197,15 +197,15 @@ def test_custom_matching_and_unpaired(H, oracle_mod):
     on the sub-rings {pair} (S=2) and {single} (S=1)."""
     import torch
     from fixtures import problem
-    S, G, P, seed = 6, 2, 20_000, 81
-    partner = [3, 1, 5, 0, 4, 2]                      # pairs (0,3), (2,5); 1 and 4 unmixed
+    S, G, P, seed = 7, 2, 20_000, 81                  # odd S: only possible with unpaired members
+    partner = [3, 1, 5, 0, 4, 2, 6]                   # pairs (0,3), (2,5); 1, 4 and 6 unmixed (T_ii = 1)
     h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
     problem.fill_weights(h, seed)
     problem.fill_grads(h, seed, 0)
     h.hadpsgd_step_matching(LR, MU, 0, partner)
     ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
     og = problem.host_grads(seed, 0, S, G, 0, P)
-    for grp in ([0, 3], [2, 5], [1], [4]):
+    for grp in ([0, 3], [2, 5], [1], [4], [6]):
         w, v, g = ow[grp].copy(), ov[grp].copy(), np.ascontiguousarray(og[grp])
         oracle_mod.step(g, w, v, LR, MU, 0)
         ow[grp], ov[grp] = w, v
@@ -214,7 +214,7 @@ def test_custom_matching_and_unpaired(H, oracle_mod):
     gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
     assert_parity(gw, gv, ow, ov, True)
     with pytest.raises(H.HadpsgdError):
-        h.hadpsgd_step_matching(LR, MU, 0, [1, 2, 0, 3, 4, 5])     # not an involution
+        h.hadpsgd_step_matching(LR, MU, 0, [1, 2, 0, 3, 4, 5, 6])  # not an involution
     h.close()
 
 
@@ -271,9 +271,12 @@ def test_diagnostics_are_run_to_run_deterministic(H):
 
 def test_error_codes(H, torch_cuda):
     torch = torch_cuda
+    odd = H.Hadpsgd(3, 2, [100])                                 # odd S > 1: no ring matching (R8) ...
     with pytest.raises(H.HadpsgdError) as e:
-        H.Hadpsgd(3, 2, [100])                                   # odd S > 1
-    assert e.value.code == -1
+        odd.hadpsgd_step(LR, MU, 0)
+    assert e.value.code == -1 and odd.hadpsgd_launch_count() == 0
+    odd.hadpsgd_step_matching(LR, MU, 0, [1, 0, 2])              # ... but a matching with T_22 = 1 is fine
+    odd.close()
     with pytest.raises(H.HadpsgdError):
         H.Hadpsgd(2, 0, [100])
     with pytest.raises(H.HadpsgdError):
@@ -337,6 +340,35 @@ def test_bf16_working_copy(H, oracle_mod, torch_cuda, bf16_grads, S, G, flagname
     with pytest.raises(H.HadpsgdError):
         plain.hadpsgd_weights_bf16(0)
     plain.close()
+
+
+def test_consensus_distance_and_variance_identity(H, oracle_mod, torch_cuda):
+    """hadpsgd_consensus: D = sum_s |w_s - wbar|^2 against the oracle, and -- with zero
+    gradients, so u = w -- the invariant D(before) - D(after) = 1/2 sum_pairs gap that ties the a5
+    pair-gap diagnostic to consensus, and the contraction of D under repeated mixing."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, seg, seed = 8, 2, ODD_TABLE, 121
+    P = sum(seg)
+    h = H.Hadpsgd(S, G, seg, H.F32, H.DETERMINISTIC)
+    problem.fill_weights(h, seed)                       # gradients and momentum stay zero
+    ow = problem.host_weights(seed, S, 0, P)
+    ov = np.zeros((S, P), np.float32)
+    og = np.zeros((S, G, P), np.float32)
+    D = [h.hadpsgd_consensus()]
+    assert D[0] == pytest.approx(oracle_mod.consensus_distance(ow), rel=1e-10)
+    for k in range(6):
+        h.hadpsgd_step(LR, MU, k)
+        d = h.hadpsgd_diagnostics()
+        oracle_mod.step(og, ow, ov, LR, MU, k)
+        D.append(h.hadpsgd_consensus())
+        assert D[-1] == pytest.approx(oracle_mod.consensus_distance(ow), rel=1e-10)
+        partner = H.hadpsgd_pairing(S, k)
+        half_gap = 0.5 * sum(d["gap"][s] for s in range(S) if s < partner[s])
+        assert D[-2] - D[-1] == pytest.approx(half_gap, rel=1e-5)
+        assert D[-1] < D[-2]
+    assert h.hadpsgd_consensus() == D[-1]               # run-to-run deterministic
+    h.close()
 
 
 def test_cuda_graph_capture_and_replay(H, oracle_mod, torch_cuda):
