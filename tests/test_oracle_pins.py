@@ -410,8 +410,9 @@ def test_invalid_arguments(oracle_mod):
 
 def _all_finite_bf16():
     bits = np.arange(65536, dtype=np.uint32)
-    vals = (bits << np.uint32(16)).view(np.float32).astype(np.float64)
-    keep = np.isfinite(vals)
+    f32 = (bits << np.uint32(16)).view(np.float32)
+    keep = np.isfinite(f32)
+    vals = np.where(keep, f32, np.float32(0)).astype(np.float64)
     return bits[keep].astype(np.uint16), vals[keep]
 
 
