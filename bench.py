@@ -34,8 +34,8 @@ LR, MU = 0.1, 0.9
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the
 # `ncu --set full` capture summarised in profiles/ (bytes; None until a capture exists)
-NCU_TRAFFIC_BYTES = {"swb2000": 74.286e9}
-NCU_TRAFFIC_SOURCE = {"swb2000": "profiles/r01_step_kernel_ncu.md (dram__bytes_read.sum 55.740 GB + dram__bytes_write.sum 18.546 GB)"}
+NCU_TRAFFIC_BYTES = {"swb2000": 74.282e9}
+NCU_TRAFFIC_SOURCE = {"swb2000": "profiles/r01_step_kernel_ncu.md (dram__bytes_read.sum 55.737 GB + dram__bytes_write.sum 18.545 GB)"}
 
 
 def parse_args():
@@ -341,7 +341,7 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dist = None
-    if world > 1:
+    if world > 1 or "RANK" in os.environ:          # launched by torch.distributed.run (any N)
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world} (launch N>1 with torch.distributed.run)"
