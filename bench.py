@@ -364,6 +364,20 @@ def run_ours(args):
     secs, clocks = time_device_steps(torch, dist, h, args.steps, args.warmup,
                                      sampler=ClockSampler(local) if rank == 0 else None)
     launches = h.hadpsgd_launch_count() - n0 - args.warmup
+    # a timed region that saw a hardware or thermal slowdown is rejected and measured again, once
+    bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+    redo = torch.tensor([1 if (clocks and bad & set(clocks["reasons"])) else 0], device="cuda")
+    if dist is not None:
+        dist.broadcast(redo, src=0)
+    remeasured = bool(int(redo[0]))
+    if remeasured:
+        time.sleep(5.0)
+        n0 = h.hadpsgd_launch_count()
+        secs, clocks = time_device_steps(torch, dist, h, args.steps, args.warmup, k0=args.steps + args.warmup,
+                                         sampler=ClockSampler(local) if rank == 0 else None)
+        launches = h.hadpsgd_launch_count() - n0 - args.warmup
+    if clocks is not None:
+        clocks["remeasured_after_slowdown"] = remeasured
     diag = None if (flags & H.NO_DIAG) else h.hadpsgd_diagnostics()
 
     e2e = None

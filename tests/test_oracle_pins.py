@@ -307,6 +307,21 @@ def test_variance_identity_links_gap_to_consensus(oracle_mod):
     assert abs((D_u - D_w) - 0.25 * d["gap"].sum()) <= 1e-6 * D_u
 
 
+def test_consensus_distance_against_two_independent_formulas(oracle_mod):
+    """D = sum_s |w_s - wbar|^2 (wbar = (1/n) sum theta^i is where mixing converges).
+    Checked against numpy's mean-based form and against the mean-free pairwise identity
+    D = (1/(2S)) sum_{s,t} |w_s - w_t|^2; zero exactly when all learners agree."""
+    for S, P in ((2, 5), (3, 64), (8, 257), (16, 33)):
+        w = rand((S, P), 70 + S, 0.05)
+        w64 = w.astype(np.float64)
+        D = oracle_mod.consensus_distance(w)
+        assert D == pytest.approx(((w64 - w64.mean(0)) ** 2).sum(), rel=1e-12)
+        pair = sum(((w64[s] - w64[t]) ** 2).sum() for s in range(S) for t in range(S)) / (2.0 * S)
+        assert D == pytest.approx(pair, rel=1e-11)
+    same = np.repeat(rand((1, 100), 3, 0.05), 6, axis=0)
+    assert oracle_mod.consensus_distance(np.ascontiguousarray(same)) == 0.0
+
+
 # ------------------------------------------------------------------ special cases (PAPER.md:72, :84)
 
 def test_ssgd_special_case(oracle_mod):
