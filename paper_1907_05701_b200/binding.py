@@ -185,7 +185,11 @@ class Hadpsgd:
         if self.arena is not None:
             off = ptr - self.arena.data_ptr()
             return self.arena[off:off + n * esz].view(dtype)
-        raise RuntimeError("views need a torch-owned arena")
+
+        class _Borrowed:      # library-owned memory: wrap the device pointer, no copy, no ownership
+            __cuda_array_interface__ = {"shape": (n * esz,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+        with torch.cuda.device(self.device):
+            return torch.as_tensor(_Borrowed(), device=self.device).view(dtype)
 
     def hadpsgd_weights(self, s):
         p = ctypes.c_void_p()

@@ -255,6 +255,36 @@ def test_host_gradient_path_equals_resident_path(H, oracle_mod):
     assert np.array_equal(bits(outs[1][0][:, lo:hi]), bits(ow))
 
 
+def test_library_owned_arena_and_two_streams(H, oracle_mod, torch_cuda):
+    """opts.arena == NULL: the library cudaMallocs (and frees) its own memory.  Two such handles on
+    two different streams run the same problem concurrently and both must match the oracle."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed = 4, 2, 200_003, 131
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    hs = []
+    for st in streams:
+        with torch.cuda.stream(st):
+            h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC, stream=st, own_arena=True)
+            assert h.arena is None
+            problem.fill_weights(h, seed)
+            problem.fill_grads(h, seed, 0)
+        hs.append(h)
+    for k in range(4):
+        for h in hs:
+            h.hadpsgd_step(LR, MU, k)           # enqueue on both streams back to back
+    torch.cuda.synchronize()
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    og = problem.host_grads(seed, 0, S, G, 0, P)
+    for k in range(4):
+        oracle_mod.step(og, ow, ov, LR, MU, k)
+    for h in hs:
+        gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+        gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+        assert_parity(gw, gv, ow, ov, True)
+        h.close()
+
+
 def test_diagnostics_are_run_to_run_deterministic(H):
     from fixtures import problem
     res = []
