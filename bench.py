@@ -296,8 +296,8 @@ def time_e2e_steps(torch, dist, h, cfg, steps, warmup=1):
     n_host = S * G
     # distinct pinned buffers for every learner when host RAM allows; otherwise one buffer per
     # learner index g shared by all super-learners (same bytes cross PCIe either way)
-    if avail and n_host * nbytes * world > 0.6 * avail:
-        n_host = G
+    if world > 1 or (avail and n_host * nbytes > 0.5 * avail):
+        n_host = G        # N ranks share one host: keep the pinned footprint at G buffers per rank
     host = []
     for b in range(n_host):
         t = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
