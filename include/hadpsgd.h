@@ -143,8 +143,9 @@ int hadpsgd_destroy(hadpsgd_handle h);
  * step_k is used only for its parity (no hidden counter: a step can be replayed).           */
 int hadpsgd_step(hadpsgd_handle h, float lr, float momentum, uint64_t step_k);
 
-/* Same step, but with a caller-supplied perfect matching (row f1): partner[s] must satisfy
- * partner[partner[s]] == s; partner[s] == s leaves s unmixed.                                */
+/* Same step, but with a caller-supplied matching (row f1): partner[s] must satisfy
+ * partner[partner[s]] == s; partner[s] == s leaves s unmixed (T_ss = 1).  A matching that has
+ * both paired and unpaired members is two launches (pairs, then singles), otherwise one.     */
 int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum, uint64_t step_k,
                           const int32_t* partner /*host [S]*/);
 

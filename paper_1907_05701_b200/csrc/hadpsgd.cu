@@ -48,6 +48,19 @@ static thread_local std::string g_create_error;
 // ---- kernel dispatch -------------------------------------------------------------------
 namespace {
 
+// Entry points that enqueue work make the handle's device current for their duration, so a
+// process that drives several GPUs may call them from any current device.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int want) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != want) switched = cudaSetDevice(want) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     if (items.empty() || elem_end <= elem_begin) return HADPSGD_OK;
@@ -142,8 +155,18 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
     const uint32_t flags = opts ? opts->flags : 0u;
     int dev = (opts && opts->device >= 0) ? opts->device : -1;
     cudaError_t e;
-    if (dev < 0) { e = cudaGetDevice(&dev); } else { e = cudaSetDevice(dev); }
-    if (e != cudaSuccess) { g_create_error = std::string("no CUDA device: ") + cudaGetErrorString(e); return HADPSGD_CUDA; }
+    if (dev < 0) {
+        e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) { g_create_error = std::string("no CUDA device: ") + cudaGetErrorString(e); return HADPSGD_CUDA; }
+    }
+    DeviceGuard guard(dev);   // the caller's current device is restored on return
+    int now = -1;
+    e = cudaGetDevice(&now);
+    if (e != cudaSuccess || now != dev) {
+        g_create_error = "cannot select CUDA device " + std::to_string(dev) + (e != cudaSuccess ? std::string(": ") + cudaGetErrorString(e) : "");
+        cudaGetLastError();
+        return HADPSGD_CUDA;
+    }
     cudaDeviceProp prop;
     e = cudaGetDeviceProperties(&prop, dev);
     if (e != cudaSuccess) { g_create_error = cudaGetErrorString(e); return HADPSGD_CUDA; }
@@ -183,6 +206,7 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
 
 extern "C" int hadpsgd_destroy(hadpsgd_handle h) {
     if (!h) return HADPSGD_INVALID_ARG;
+    DeviceGuard guard(h->device);
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t ev : h->chunk_events) cudaEventDestroy(ev);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -198,6 +222,7 @@ extern "C" int hadpsgd_step(hadpsgd_handle h, float lr, float momentum, uint64_t
 extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum, uint64_t step_k,
                                      const int32_t* partner) {
     if (!h) return HADPSGD_INVALID_ARG;
+    DeviceGuard guard(h->device);
     std::vector<int32_t> pt;
     int rc = build_partner(h, step_k, partner, &pt);
     if (rc != HADPSGD_OK) return rc;
@@ -208,6 +233,7 @@ extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum,
 extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads, float lr,
                                  float momentum, uint64_t step_k, hadpsgd_diag* diag_out) {
     if (!h || !host_grads) return HADPSGD_INVALID_ARG;
+    DeviceGuard guard(h->device);
     std::vector<int32_t> pt;
     int rc = build_partner(h, step_k, nullptr, &pt);
     if (rc != HADPSGD_OK) return rc;
@@ -282,6 +308,7 @@ extern "C" int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded) {
 extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
     if (!h || !host_out) return HADPSGD_INVALID_ARG;
     if (h->flags & HADPSGD_NO_DIAG) { h->err = "handle was created with HADPSGD_NO_DIAG"; return HADPSGD_INVALID_ARG; }
+    DeviceGuard guard(h->device);
     const int S = h->L.S;
     std::vector<double> tmp(3 * S);
     CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * 3 * S, cudaMemcpyDeviceToHost, h->stream));
@@ -300,6 +327,7 @@ int launch_consensus(const float* w, long long P_padded, int S, int num_sms, dou
 
 extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
     if (!h || !D_out) return HADPSGD_INVALID_ARG;
+    DeviceGuard guard(h->device);
     // the partials scratch is free between steps: everything is ordered on h->stream
     cudaError_t e = cudaSuccess;
     const int grid = launch_consensus(reinterpret_cast<const float*>(h->arena + h->L.w_off), h->L.P_padded, h->L.S,
