@@ -255,6 +255,54 @@ def test_host_gradient_path_equals_resident_path(H, oracle_mod):
     assert np.array_equal(bits(outs[1][0][:, lo:hi]), bits(ow))
 
 
+@pytest.mark.parametrize("exact", [True, False])
+def test_special_values_propagate_like_ieee(H, oracle_mod, torch_cuda, exact):
+    """DESIGN.md R17: no flush-to-zero, Inf/NaN propagate.  Subnormal weights, momenta and gradients,
+    huge values whose pair sum overflows, Inf and NaN are planted in both sides' inputs; finite
+    results must match (bit for bit in deterministic mode), NaN and Inf must land in the same
+    places."""
+    torch = torch_cuda
+    S, G, P = 4, 2, 4096
+    rng = np.random.default_rng(7)
+    w = (rng.standard_normal((S, P)) * 0.05).astype(np.float32)
+    v = (rng.standard_normal((S, P)) * 0.01).astype(np.float32)
+    g = (rng.standard_normal((S, G, P)) * 1e-3).astype(np.float32)
+    sub = np.float32(1e-45)                                  # smallest subnormal
+    w[0, 0:8] = [sub, -sub, 3 * sub, 1e-39, -1e-39, 0.0, -0.0, 1.1754942e-38]
+    w[1:, 0:8] = w[0, 0:8]; v[:, 0:8] = 0.0; g[:, :, 0:8] = 0.0      # every pair averages equal subnormals
+    g[2, :, 8:16] = sub; v[2, 8:16] = 2 * sub                # subnormal gradient mean and momentum
+    w[0, 16], w[1, 16] = 3.0e38, 3.0e38                      # u_s + u_p overflows to +Inf before the 1/2
+    w[2, 17] = np.inf; w[3, 18] = -np.inf; w[0, 19] = np.nan; g[1, 0, 20] = np.nan; v[3, 21] = np.inf
+    g[2, 1, 22] = np.inf; g[2, 0, 22] = -np.inf             # Inf - Inf in the learner sum -> NaN
+    h = H.Hadpsgd(S, G, [P], H.F32, (H.DETERMINISTIC if exact else 0))
+    for s in range(S):
+        h.hadpsgd_weights(s)[:P] = torch.from_numpy(w[s]).cuda()
+        h.hadpsgd_momentum(s)[:P] = torch.from_numpy(v[s]).cuda()
+        for k in range(G):
+            h.hadpsgd_grads(s, k)[:P] = torch.from_numpy(g[s, k]).cuda()
+    ow, ov = w.copy(), v.copy()
+    with np.errstate(all="ignore"):
+        for k in range(2):
+            h.hadpsgd_step(LR, MU, k)
+            oracle_mod.step(g, ow, ov, LR, MU, k)
+    torch.cuda.synchronize()
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    h.close()
+    for got, want in ((gw, ow), (gv, ov)):
+        assert np.array_equal(np.isnan(got), np.isnan(want))
+        assert np.array_equal(np.isposinf(got), np.isposinf(want)) and np.array_equal(np.isneginf(got), np.isneginf(want))
+        fin = np.isfinite(want)
+        if exact:
+            assert np.array_equal(bits(got)[fin], bits(want)[fin])
+        else:
+            with np.errstate(all="ignore"):
+                assert np.all(np.abs(got[fin] - want[fin]) <= 1e-6 + 1e-5 * np.abs(want[fin]))
+    assert np.isnan(ow).sum() >= 3 and np.isinf(ow).sum() >= 3          # the plants did propagate
+    # subnormal inputs were not flushed: 1/2 (sub + sub) = sub, 1/2 (3 sub + 3 sub) = 3 sub
+    assert gw[0, 0] == sub and gw[0, 2] == 3 * sub and gw[0, 1] == -sub
+
+
 def test_library_owned_arena_and_two_streams(H, oracle_mod, torch_cuda):
     """opts.arena == NULL: the library cudaMallocs (and frees) its own memory.  Two such handles on
     two different streams run the same problem concurrently and both must match the oracle."""
