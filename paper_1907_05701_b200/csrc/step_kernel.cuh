@@ -223,8 +223,10 @@ __device__ __forceinline__ double warp_sum(double x) {
 // issued before any is consumed).  G == 0: runtime learner count.
 // Persistent grid: gridDim.x = (#SMs x resident blocks/SM); block b walks global tiles b,
 // b+grid, ... of the item-major (work item, tile) space ("pair-major": for large P the whole
-// chip streams the same 2G+4 read streams and 4 write streams at any moment, which keeps DRAM
-// pages open; for small P the items spread over the blocks instead of serialising).  A tile is
+// chip streams the same 2G+4 read streams and 4 write streams at any moment, so few 2 MB pages
+// and DRAM rows are live at once -- giving each block one contiguous range instead measured
+// 2-10 % slower at 2^20..2^26 parameters; for small P the items spread over the blocks instead
+// of serialising).  A tile is
 // THREADS x U units; thread t owns units t, t+THREADS, ... of the tile, so each warp request
 // covers 1 KB contiguous of one stream.
 // ---------------------------------------------------------------------------------------
