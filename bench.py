@@ -53,7 +53,7 @@ def parse_args():
     ap.add_argument("--cpu-sample-elems", type=int, default=1 << 22)
     ap.add_argument("--cpu-sample-steps", type=int, default=20)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
-    ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7")
+    ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7,share")
     ap.add_argument("--emit-bf16", action="store_true",
                     help="also write the bf16 working copy of the weights every step (row f2; +2 B/param)")
     ap.add_argument("--sweep", action="store_true",
@@ -250,7 +250,8 @@ def run_reference(args):
 # ------------------------------------------------------------------ the GPU arm
 
 def parse_flags(H, text):
-    table = {"deterministic": H.DETERMINISTIC, "no_diag": H.NO_DIAG, "no_mix": H.NO_MIX, "eq7": H.EQ7_LITERAL}
+    table = {"deterministic": H.DETERMINISTIC, "no_diag": H.NO_DIAG, "no_mix": H.NO_MIX, "eq7": H.EQ7_LITERAL,
+             "share": H.SHARE_PAIR_WEIGHTS}
     flags = 0
     for name in filter(None, (t.strip() for t in text.split(","))):
         flags |= table[name]

@@ -57,7 +57,13 @@ enum { /* hadpsgd_opts.flags */
                                         g=0..G-1: w and v are BIT-EXACT against the oracle               */
     HADPSGD_NO_MIX        = 1u << 1, /* T_k = I: eq. (6)/(3) only, every super-learner keeps u_s         */
     HADPSGD_NO_DIAG       = 1u << 2, /* skip a5                                                          */
-    HADPSGD_EQ7_LITERAL   = 1u << 3  /* eq. (7) as printed: w'_s = 1/2 (w_s + w_p) - lr v_s  (row f1)    */
+    HADPSGD_EQ7_LITERAL   = 1u << 3, /* eq. (7) as printed: w'_s = 1/2 (w_s + w_p) - lr v_s  (row f1)    */
+    HADPSGD_SHARE_PAIR_WEIGHTS = 1u << 4 /* both members of a pair end a step with identical weights (R3),
+                                        so they SHARE one of the S weight buffers: one weight write per
+                                        pair instead of two, and the buffer two neighbouring pairs read
+                                        next step is fetched from HBM once.  Same arithmetic, same
+                                        results; what changes is which buffer hadpsgd_weights(h, s)
+                                        points to (see there).  Not with NO_MIX or EQ7_LITERAL.          */
 };
 
 #define HADPSGD_SEG_ALIGN_ELEMS 64 /* 256 B in fp32, 128 B in bf16 */
@@ -156,8 +162,22 @@ int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum, uint64_t s
 int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads /*host [S*G]*/,
                       float lr, float momentum, uint64_t step_k, hadpsgd_diag* diag_out);
 
-/* accessors (borrowed device pointers; no copy, no sync) ------------------------------------- */
+/* accessors (borrowed device pointers; no copy, no sync) -------------------------------------
+ * Without HADPSGD_SHARE_PAIR_WEIGHTS every pointer is fixed for the life of the handle.  With it,
+ * hadpsgd_weights / hadpsgd_weights_bf16 return the buffer that holds w_s NOW: it is valid until
+ * the next hadpsgd_step* call, pair members return the same pointer, and weights must only be
+ * written through it before the first step or after hadpsgd_unshare().                        */
 int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr);
+/* Gives every super-learner a weight buffer of its own again (copies the shared ones on the
+ * stream; asynchronous).  A no-op without HADPSGD_SHARE_PAIR_WEIGHTS or before the first step. */
+int hadpsgd_unshare(hadpsgd_handle h);
+/* The slot assignment of one step as a pure host function (what hadpsgd_step* does internally):
+ * partner [S] is a matching; w_slot [S] in/out = buffer index holding w_s before / after the step;
+ * read_slot [S] / write_slot [S] = buffer each member's weights are read from / written to;
+ * copy_src / copy_dst [S] receive the *n_copies un-sharing copies that must run first (only when
+ * the matching has unmixed members).  share = 0 gives the identity everywhere.                 */
+int hadpsgd_plan_slots(int S, const int32_t* partner, int share, int32_t* w_slot, int32_t* read_slot,
+                       int32_t* write_slot, int32_t* copy_src, int32_t* copy_dst, int32_t* n_copies);
 int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr);
 int hadpsgd_grads(hadpsgd_handle h, int s, int g, void** dev_ptr);
 /* bf16 working copy of super-learner s's weights (P_padded bf16 values, rewritten by every step;

@@ -11,7 +11,7 @@ import numpy as np
 
 F32, BF16 = 0, 1
 OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_DEVICE = 0, -1, -2, -3, -4
-DETERMINISTIC, NO_MIX, NO_DIAG, EQ7_LITERAL = 1, 2, 4, 8
+DETERMINISTIC, NO_MIX, NO_DIAG, EQ7_LITERAL, SHARE_PAIR_WEIGHTS = 1, 2, 4, 8, 16
 SEG_ALIGN_ELEMS = 64
 MAX_S = 512
 
@@ -70,6 +70,9 @@ def lib():
         L.hadpsgd_segment.argtypes = [vp, i32, i64p, i64p]
         L.hadpsgd_padded_len.argtypes = [vp, i64p]
         L.hadpsgd_diagnostics.argtypes = [vp, ctypes.POINTER(hadpsgd_diag)]
+        i32p = ctypes.POINTER(ctypes.c_int32)
+        L.hadpsgd_unshare.argtypes = [vp]
+        L.hadpsgd_plan_slots.argtypes = [i32, i32p, i32, i32p, i32p, i32p, i32p, i32p, i32p]
         L.hadpsgd_consensus.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
         L.hadpsgd_set_launch.argtypes = [vp, i32]
         L.hadpsgd_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
@@ -127,6 +130,16 @@ def hadpsgd_lr_schedule(base_lr, base_batch, total_batch, warmup_epochs, epoch):
     out = ctypes.c_double(0.0)
     _check(lib().hadpsgd_lr_schedule(base_lr, base_batch, total_batch, warmup_epochs, epoch, ctypes.byref(out)))
     return out.value
+
+
+def hadpsgd_plan_slots(partner, w_slot, share=True):
+    """Pure host function: (w_slot_after, read_slot, write_slot, copies[(src, dst)...]) of one step."""
+    S = len(partner)
+    arr = lambda v: (ctypes.c_int32 * S)(*[int(x) for x in v])
+    pt, ws, rd, wr, cs, cd = arr(partner), arr(w_slot), arr([0] * S), arr([0] * S), arr([0] * S), arr([0] * S)
+    n = ctypes.c_int32(0)
+    _check(lib().hadpsgd_plan_slots(S, pt, 1 if share else 0, ws, rd, wr, cs, cd, ctypes.byref(n)))
+    return list(ws), list(rd), list(wr), [(cs[i], cd[i]) for i in range(n.value)]
 
 
 class Hadpsgd:
@@ -231,6 +244,9 @@ class Hadpsgd:
         d = hadpsgd_diag()
         _check(lib().hadpsgd_diagnostics(self.h, ctypes.byref(d)), self.h)
         return self._diag_dict(d)
+
+    def hadpsgd_unshare(self):
+        _check(lib().hadpsgd_unshare(self.h), self.h)
 
     def hadpsgd_consensus(self):
         out = ctypes.c_double(0.0)

@@ -22,6 +22,8 @@ struct hadpsgd_ctx {
     cudaStream_t copy_stream = nullptr;   // host path: H2D copies overlap the kernel
     std::vector<cudaEvent_t> chunk_events;
     std::vector<std::pair<const void*, int>> occupancy;   // per kernel instantiation, queried once
+    std::vector<std::pair<const void*, size_t>> smem_optin; // largest dynamic smem opted in per kernel
+    std::vector<int32_t> w_slot;                           // slot (buffer index) that holds w_s right now
     char* arena = nullptr;
     bool owns_arena = false;
     double* d_partials = nullptr;
@@ -61,9 +63,8 @@ struct DeviceGuard {
     DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
-int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, float lr, float mu,
+int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, bool tile_major, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
-    if (items.empty() || elem_end <= elem_begin) return HADPSGD_OK;
     const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
     const bool exact = h->flags & HADPSGD_DETERMINISTIC;
     const bool diag = !(h->flags & HADPSGD_NO_DIAG);
@@ -81,13 +82,15 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
     a.unit_begin = elem_begin / unit;
     a.unit_end = elem_end / unit;
     a.G = h->L.G;
-    a.n_work = static_cast<int>(items.size());
+    a.n_work = n_items;
     a.lr = lr; a.mu = mu;
     a.invG = 1.0f / static_cast<float>(h->L.G);   // fp32 reciprocal, exact for G = 1,2,4,8 (R5)
     a.accumulate_diag = accumulate ? 1 : 0;
     a.S = h->L.S;
     a.partials = h->d_partials; a.diag = h->d_diag; a.ticket = h->d_ticket;
-    for (size_t j = 0; j < items.size(); ++j) a.work[j] = make_short2(static_cast<short>(items[j].a), static_cast<short>(items[j].b));
+    a.tile_major = tile_major ? 1 : 0;
+    for (int j = 0; j < n_items; ++j)
+        a.work[j] = pack_item(items[j].s, items[j].p, items[j].ws, items[j].wp, items[j].wo_s, items[j].wo_p);
 
     int occ = 0;
     for (const auto& kv : h->occupancy) if (kv.first == plan.fn) occ = kv.second;
@@ -95,6 +98,16 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
         CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, 0));
         if (occ < 1) occ = 1;
         h->occupancy.emplace_back(plan.fn, occ);
+    }
+    // per-warp diagnostic accumulators: [warps][items][5] doubles of dynamic shared memory
+    const size_t smem = diag ? static_cast<size_t>(plan.threads / 32) * n_items * kDiagQuantities * sizeof(double) : 0;
+    if (smem > 48 * 1024) {
+        size_t have = 0;
+        for (const auto& kv : h->smem_optin) if (kv.first == plan.fn) have = kv.second;
+        if (have < smem) {
+            CUDA_TRY(h, cudaFuncSetAttribute(plan.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+            h->smem_optin.emplace_back(plan.fn, smem);
+        }
     }
     int bps = h->blocks_per_sm > 0 ? h->blocks_per_sm : plan.blocks_per_sm;
     if (bps > occ) bps = occ;                      // persistent grid: never more than fit at once
@@ -106,22 +119,60 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, f
     if (grid < 1) grid = 1;
 
     void* params[] = {&a};
-    CUDA_TRY(h, cudaLaunchKernel(plan.fn, dim3(static_cast<unsigned>(grid)), dim3(plan.threads), params, 0, h->stream));
+    CUDA_TRY(h, cudaLaunchKernel(plan.fn, dim3(static_cast<unsigned>(grid)), dim3(plan.threads), params, smem, h->stream));
     h->launches++;
     return HADPSGD_OK;
 }
 
-// One step over [elem_begin, elem_end) for an arbitrary matching.
-int step_range(hadpsgd_ctx* h, const int32_t* partner, float lr, float mu, int64_t elem_begin,
-               int64_t elem_end, bool accumulate) {
-    std::vector<WorkItem> pairs, singles;
-    matching_to_work(h->L.S, partner, &pairs, &singles);
-    h->last_n_pairs = static_cast<int>(pairs.size());
+// All items of one mode over [elem_begin, elem_end); more than kMaxWork items (S > 480 unmixed
+// super-learners) take several launches.
+int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, bool tile_major, float lr, float mu,
+                 int64_t elem_begin, int64_t elem_end, bool accumulate) {
+    if (elem_end <= elem_begin) return HADPSGD_OK;
+    for (size_t first = 0; first < items.size(); first += kMaxWork) {
+        const int n = static_cast<int>(items.size() - first < static_cast<size_t>(kMaxWork) ? items.size() - first : kMaxWork);
+        int rc = launch_chunk(h, items.data() + first, n, mode, tile_major, lr, mu, elem_begin, elem_end, accumulate);
+        if (rc != HADPSGD_OK) return rc;
+    }
+    return HADPSGD_OK;
+}
+
+// The launches of one step over the element range [elem_begin, elem_end).
+struct StepPlan { std::vector<WorkItem> pairs, singles; bool shared = false; };
+
+int step_range(hadpsgd_ctx* h, const StepPlan& sp, float lr, float mu, int64_t elem_begin, int64_t elem_end,
+               bool accumulate) {
     const int pair_mode = (h->flags & HADPSGD_EQ7_LITERAL) ? kPairEq7 : kPair;
-    int rc = launch_items(h, pairs, pair_mode, lr, mu, elem_begin, elem_end, accumulate);
+    int rc = launch_items(h, sp.pairs, pair_mode, sp.shared, lr, mu, elem_begin, elem_end, accumulate);
     if (rc != HADPSGD_OK) return rc;
     // unmixed super-learners (S == 1, NO_MIX, or partner[s] == s in a custom matching)
-    return launch_items(h, singles, kSingle, lr, mu, elem_begin, elem_end, accumulate);
+    return launch_items(h, sp.singles, kSingle, false, lr, mu, elem_begin, elem_end, accumulate);
+}
+
+// Copies weight slot src to slot dst (and the bf16 working copy with it) on the handle's stream.
+int copy_slots(hadpsgd_ctx* h, const std::vector<SlotCopy>& copies) {
+    for (const SlotCopy& c : copies) {
+        char* wbase = h->arena + h->L.w_off;
+        CUDA_TRY(h, cudaMemcpyAsync(wbase + static_cast<size_t>(c.dst) * h->L.w_stride_bytes(),
+                                    wbase + static_cast<size_t>(c.src) * h->L.w_stride_bytes(), h->L.w_stride_bytes(),
+                                    cudaMemcpyDeviceToDevice, h->stream));
+        if (h->L.working_dtype == HADPSGD_BF16) {
+            char* bbase = h->arena + h->L.wb_off;
+            const size_t nb = static_cast<size_t>(h->L.P_padded) * 2;
+            CUDA_TRY(h, cudaMemcpyAsync(bbase + c.dst * nb, bbase + c.src * nb, nb, cudaMemcpyDeviceToDevice, h->stream));
+        }
+    }
+    return HADPSGD_OK;
+}
+
+// Matching -> work items with weight slots (updates h->w_slot) and enqueues any un-sharing copies.
+int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp) {
+    const bool share = h->flags & HADPSGD_SHARE_PAIR_WEIGHTS;
+    std::vector<SlotCopy> copies;
+    plan_step(h->L.S, partner, share, &h->w_slot, &sp->pairs, &sp->singles, &copies);
+    sp->shared = share;
+    h->last_n_pairs = static_cast<int>(sp->pairs.size());
+    return copy_slots(h, copies);
 }
 
 int build_partner(hadpsgd_ctx* h, uint64_t step_k, const int32_t* custom, std::vector<int32_t>* partner) {
@@ -175,7 +226,14 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
         return HADPSGD_UNSUPPORTED_DEVICE;
     }
 
+    if ((flags & HADPSGD_SHARE_PAIR_WEIGHTS) && (flags & (HADPSGD_NO_MIX | HADPSGD_EQ7_LITERAL))) {
+        g_create_error = "HADPSGD_SHARE_PAIR_WEIGHTS needs pair members that end a step with identical weights: "
+                         "not with NO_MIX or EQ7_LITERAL";
+        return HADPSGD_INVALID_ARG;
+    }
     hadpsgd_ctx* h = new hadpsgd_ctx();
+    h->w_slot.resize(S);
+    for (int s = 0; s < S; ++s) h->w_slot[s] = s;
     h->L = L; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount;
     h->stream = opts ? static_cast<cudaStream_t>(opts->stream) : nullptr;
     if (opts && opts->arena) {
@@ -227,7 +285,10 @@ extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum,
     int rc = build_partner(h, step_k, partner, &pt);
     if (rc != HADPSGD_OK) return rc;
     h->last_step_k = step_k;
-    return step_range(h, pt.data(), lr, momentum, 0, h->L.P_padded, false);
+    StepPlan sp;
+    rc = plan_and_prepare(h, pt.data(), &sp);
+    if (rc != HADPSGD_OK) return rc;
+    return step_range(h, sp, lr, momentum, 0, h->L.P_padded, false);
 }
 
 extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads, float lr,
@@ -240,6 +301,10 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
     h->last_step_k = step_k;
     const int n_buf = h->L.S * h->L.G;
     for (int b = 0; b < n_buf; ++b) if (!host_grads[b]) { h->err = "host_grads[] has a NULL entry"; return HADPSGD_INVALID_ARG; }
+
+    StepPlan sp;                      // one slot plan for the whole step, shared by all chunks
+    rc = plan_and_prepare(h, pt.data(), &sp);
+    if (rc != HADPSGD_OK) return rc;
 
     // Chunk the element range so the H2D copy of chunk c+1 overlaps the kernel on chunk c.
     const int64_t P = h->L.P_padded;
@@ -264,7 +329,7 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
                                         static_cast<size_t>(e1 - e0) * eb, cudaMemcpyHostToDevice, h->copy_stream));
         CUDA_TRY(h, cudaEventRecord(h->chunk_events[c], h->copy_stream));
         CUDA_TRY(h, cudaStreamWaitEvent(h->stream, h->chunk_events[c], 0));
-        rc = step_range(h, pt.data(), lr, momentum, e0, e1, c > 0);
+        rc = step_range(h, sp, lr, momentum, e0, e1, c > 0);
         if (rc != HADPSGD_OK) return rc;
     }
     if (diag_out) return hadpsgd_diagnostics(h, diag_out);
@@ -274,7 +339,7 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
 
 extern "C" int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr) {
     if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
-    *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.w_off + static_cast<size_t>(s) * h->L.w_stride_bytes());
+    *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.w_off + static_cast<size_t>(h->w_slot[s]) * h->L.w_stride_bytes());
     return HADPSGD_OK;
 }
 extern "C" int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr) {
@@ -285,7 +350,7 @@ extern "C" int hadpsgd_momentum(hadpsgd_handle h, int s, float** dev_ptr) {
 extern "C" int hadpsgd_weights_bf16(hadpsgd_handle h, int s, void** dev_ptr) {
     if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
     if (h->L.working_dtype != HADPSGD_BF16) { h->err = "handle was created without a bf16 working copy (dtypes.working_dtype)"; return HADPSGD_INVALID_ARG; }
-    *dev_ptr = h->arena + h->L.wb_off + static_cast<size_t>(s) * static_cast<size_t>(h->L.P_padded) * 2;
+    *dev_ptr = h->arena + h->L.wb_off + static_cast<size_t>(h->w_slot[s]) * static_cast<size_t>(h->L.P_padded) * 2;
     return HADPSGD_OK;
 }
 extern "C" int hadpsgd_grads(hadpsgd_handle h, int s, int g, void** dev_ptr) {
@@ -321,8 +386,16 @@ extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
 }
 
 namespace hadpsgd {
-int launch_consensus(const float* w, long long P_padded, int S, int num_sms, double* block_out,
-                     cudaStream_t stream, cudaError_t* err);   // consensus.cu
+int launch_consensus(const float* w, long long P_padded, int S, const int32_t* w_slot, int num_sms,
+                     double* block_out, cudaStream_t stream, cudaError_t* err);   // consensus.cu
+}
+
+extern "C" int hadpsgd_unshare(hadpsgd_handle h) {
+    if (!h) return HADPSGD_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    std::vector<SlotCopy> copies;
+    plan_unshare(h->L.S, &h->w_slot, &copies);
+    return copy_slots(h, copies);
 }
 
 extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
@@ -331,7 +404,7 @@ extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
     // the partials scratch is free between steps: everything is ordered on h->stream
     cudaError_t e = cudaSuccess;
     const int grid = launch_consensus(reinterpret_cast<const float*>(h->arena + h->L.w_off), h->L.P_padded, h->L.S,
-                                      h->num_sms, h->d_partials, h->stream, &e);
+                                      h->w_slot.data(), h->num_sms, h->d_partials, h->stream, &e);
     CUDA_TRY(h, e);
     h->launches++;
     std::vector<double> part(grid);

@@ -37,12 +37,32 @@ constexpr int kDiagQuantities = 5;  // per work item: gsq_s, gsq_p, wsq_s, wsq_p
 int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
                    Layout* out, std::string* err);
 
-// a1: work list for one step.  Each item is (a, b): a pair to average, or a == b (unmixed).
-struct WorkItem { int32_t a, b; };
+// a1: work list for one step.  Each item is a pair (s, p) to average, or s == p (unmixed).
+// ws / wp: weight SLOT (buffer index 0..S-1) that currently holds w_s / w_p; wo_s / wo_p: slot the
+// new weights of s / p are written to.  Without HADPSGD_SHARE_PAIR_WEIGHTS every slot is the
+// member's own index.  With it both members of a pair share ONE slot (wo_s == wo_p), because
+// they hold identical bits after the step (R3): one weight write instead of two.
+struct WorkItem { int32_t s, p, ws, wp, wo_s, wo_p; };
+struct SlotCopy { int32_t src, dst; };   // "copy weight slot src to slot dst" (un-sharing)
+
 int ring_partner(int S, uint64_t step_k, int32_t* partner);  // even/odd ring pairing
 int validate_matching(int S, const int32_t* partner);        // partner[partner[s]] == s
-// Splits a matching into pair items (a < b) and single items (a == b), in ascending a.
-void matching_to_work(int S, const int32_t* partner, std::vector<WorkItem>* pairs,
-                      std::vector<WorkItem>* singles);
+
+// Turns a matching into pair items (s < p) and single items (s == p), ascending s, and assigns
+// weight slots.  w_slot[s] (in/out, [S]) = slot holding w_s before / after the step.
+//   share == false: slots are the identity, w_slot is left untouched.
+//   share == true : (1) if the matching has unmixed members while some slot is shared, the shared
+//                   slots are first split again (copies: src -> a free slot);
+//                   (2) every pair writes to ONE slot that no other item of this step reads:
+//                   in place if one member's current slot is referenced by nobody outside the
+//                   pair, else the lowest-numbered slot that is free at the start of the step.
+// A free slot always exists when needed: S slots, S members, so the number of free slots equals
+// the number of shared ones, and a pair needs a free slot only if both its members come out of
+// two different shared slots.
+void plan_step(int S, const int32_t* partner, bool share, std::vector<int32_t>* w_slot,
+               std::vector<WorkItem>* pairs, std::vector<WorkItem>* singles,
+               std::vector<SlotCopy>* copies);
+// Splits every shared slot (copies: src -> free slot); afterwards w_slot is injective.
+void plan_unshare(int S, std::vector<int32_t>* w_slot, std::vector<SlotCopy>* copies);
 
 }  // namespace hadpsgd

@@ -14,9 +14,10 @@
 // each byte is touched exactly once, so the design goal is only "the right amount of coalesced
 // 32 B requests in flight per SM" (~100 KB) and full-sector writes.
 //
-// Diagnostics: per-thread double accumulators -> warp shuffle tree -> block partial in a
-// fixed slot of global scratch (no atomics on data) -> the last block to finish (ticket)
-// reduces the partials in a fixed order.  Results are therefore run-to-run deterministic.
+// Diagnostics: per tile, per-thread sums -> warp shuffle tree -> the warp's own accumulator of
+// that work item in shared memory (no atomics, no block barrier per tile) -> at the end one block
+// partial per item in a fixed slot of global scratch -> the last block to finish (ticket) reduces
+// the partials in a fixed order.  Results are therefore run-to-run deterministic.
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -24,7 +25,7 @@
 
 namespace hadpsgd {
 
-constexpr int kMaxWork = 512;
+constexpr int kMaxWork = 480;   // work items per launch: 480 x 8 B keeps StepArgs under 4 KB
 constexpr int kNQ = 5;  // gsq_a, gsq_b, wsq_a, wsq_b, gap
 
 enum Mode : int { kPair = 0, kSingle = 1, kPairEq7 = 2 };
@@ -45,8 +46,23 @@ struct StepArgs {
     double* partials;     // [n_work][kNQ][gridDim.x]
     double* diag;         // gsq[S] | wsq[S] | gap[S]
     unsigned int* ticket;
-    short2 work[kMaxWork];
+    int tile_major;       // 0: item-major tile walk; 1: tile-major (all items of a tile, then the next)
+    unsigned long long work[kMaxWork];   // six 10-bit fields per item, see pack_item()
 };
+
+// Work item = (s, p, ws, wp, wo_s, wo_p): super-learner indices of the pair (gradients and
+// momentum are always indexed by s / p), the weight slots w_s / w_p are READ from, and the slots
+// the new weights are WRITTEN to (wo_s == wo_p when the pair shares one copy).  S <= 512.
+__host__ __device__ inline unsigned long long pack_item(int s, int p, int ws, int wp, int wo_s, int wo_p) {
+    return static_cast<unsigned long long>(s) | static_cast<unsigned long long>(p) << 10 |
+           static_cast<unsigned long long>(ws) << 20 | static_cast<unsigned long long>(wp) << 30 |
+           static_cast<unsigned long long>(wo_s) << 40 | static_cast<unsigned long long>(wo_p) << 50;
+}
+struct Item { int s, p, ws, wp, wo_s, wo_p; };
+__device__ __forceinline__ Item unpack_item(unsigned long long w) {
+    return {static_cast<int>(w & 1023u), static_cast<int>((w >> 10) & 1023u), static_cast<int>((w >> 20) & 1023u),
+            static_cast<int>((w >> 30) & 1023u), static_cast<int>((w >> 40) & 1023u), static_cast<int>((w >> 50) & 1023u)};
+}
 
 // ---- memory access helpers -------------------------------------------------------------
 // Every byte is touched once per step, so all traffic is issued as 32-byte vector accesses
@@ -236,7 +252,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     constexpr int GA = G > 0 ? G : 1;
     constexpr bool PAIRED = (MODE != kSingle);
     constexpr int NP = PAIRED ? U : 1;   // array extent of the partner's registers
-    __shared__ double s_red[THREADS / 32][kNQ];
+    constexpr int WARPS = THREADS / 32;
+    extern __shared__ double s_acc[];    // DIAG: [WARPS][n_work][kNQ], each warp owns its rows
     __shared__ unsigned int s_last;
 
     const int tid = threadIdx.x;
@@ -246,45 +263,50 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     const char* gbytes = static_cast<const char*>(a.g);
     constexpr long long TILE = static_cast<long long>(THREADS) * U;
 
-    // a5: flush this block's partial sums of work item j to its fixed slot partials[j][q][block]
+    if constexpr (DIAG) {
+        for (int idx = tid; idx < WARPS * a.n_work * kNQ; idx += THREADS) s_acc[idx] = 0.;
+        __syncthreads();
+    }
+
+    // Flattened (work item, tile) space; block b takes global tiles b, b+grid, ...
+    //  item-major: tiles of item 0, then item 1, ...: for large P the whole chip streams one pair
+    //              at a time (few 2 MB pages and DRAM rows live at once).
+    //  tile-major: all items of tile 0, then tile 1, ...: used when pairs share weight slots --
+    //              the slot two neighbouring pairs both read is then fetched from HBM once and
+    //              hits in L2 the second time.
+    const long long n_tiles = (n_units + TILE - 1) / TILE;
+    const long long total_tiles = n_tiles * a.n_work;
+    // a5: per-thread sums of the item being worked on; when the block moves to another item they
+    // go through a warp shuffle tree into the warp's own accumulator row of the old item (no
+    // block barrier).  (Placing the hand-over after the next tile's loads, to hide its latency,
+    // keeps all loads live across the shuffles and costs registers -- measured slower.)
     double d_gs = 0., d_gp = 0., d_ws = 0., d_wp = 0., d_gap = 0.;
-    auto flush = [&](int j) {
+    int cur = -1;
+    Item it = {0, 0, 0, 0, 0, 0};
+    auto hand_over = [&](int item) {
         if constexpr (MODE == kPair) d_wp = d_ws;
         double q[kNQ] = {d_gs, d_gp, d_ws, d_wp, d_gap};
 #pragma unroll
         for (int k = 0; k < kNQ; ++k) q[k] = warp_sum(q[k]);
-        if ((tid & 31) == 0)
+        if ((tid & 31) == 0) {
+            double* row = s_acc + (static_cast<size_t>(tid >> 5) * a.n_work + item) * kNQ;
 #pragma unroll
-            for (int k = 0; k < kNQ; ++k) s_red[tid >> 5][k] = q[k];
-        __syncthreads();
-        if (tid < kNQ) {
-            double tot = 0.;
-            for (int wi = 0; wi < THREADS / 32; ++wi) tot += s_red[wi][tid];  // fixed order
-            a.partials[(static_cast<size_t>(j) * kNQ + tid) * gridDim.x + blockIdx.x] = tot;
+            for (int k = 0; k < kNQ; ++k) row[k] += q[k];
         }
-        __syncthreads();
         d_gs = d_gp = d_ws = d_wp = d_gap = 0.;
     };
-    if constexpr (DIAG) {
-        // slots of work items this block never touches (small problems) must read as zero
-        for (int idx = tid; idx < a.n_work * kNQ; idx += THREADS)
-            a.partials[static_cast<size_t>(idx) * gridDim.x + blockIdx.x] = 0.;
-        __syncthreads();
-    }
-
-    // Flattened (work item, tile) space, item-major: block b takes global tiles b, b+grid, ...
-    // For large P every block walks all items in order (the whole chip streams one pair at a
-    // time); for small P the items spread over the blocks instead of serialising.
-    const long long n_tiles = (n_units + TILE - 1) / TILE;
-    const long long total_tiles = n_tiles * a.n_work;
-    int cur = -1, s = 0, p = 0;
     for (long long gt = blockIdx.x; gt < total_tiles; gt += gridDim.x) {
-        const int j = static_cast<int>(gt / n_tiles);
-        const long long base = (gt - static_cast<long long>(j) * n_tiles) * TILE;
-        if (j != cur) {                       // block-uniform: every thread sees the same gt
-            if constexpr (DIAG) { if (cur >= 0) flush(cur); }
-            cur = j; s = a.work[j].x; p = a.work[j].y;
+        int j;
+        long long tile;
+        if (a.tile_major) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
+        else { j = static_cast<int>(gt / n_tiles); tile = gt - static_cast<long long>(j) * n_tiles; }
+        const long long base = tile * TILE;
+        if (j != cur) {                                  // block-uniform
+            if constexpr (DIAG) { if (cur >= 0) hand_over(cur); }
+            cur = j;
+            it = unpack_item(a.work[j]);
         }
+        const int s = it.s, p = it.p;
         {
             Vec<UNIT> ws[U], vs[U], gbs[U], wp[NP], vp[NP], gbp[NP];
             bool live[U];
@@ -304,10 +326,10 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     if (live[q]) {
                         load_grads<GA, BF16>(gbytes, P, s, elem[q], grs[q]);
                         if constexpr (PAIRED) load_grads<GA, BF16>(gbytes, P, p, elem[q], grp[q]);
-                        load_state<UNIT>(a.w, static_cast<long long>(s) * P + elem[q], ws[q]);
+                        load_state<UNIT>(a.w, static_cast<long long>(it.ws) * P + elem[q], ws[q]);
                         load_state<UNIT>(a.v, static_cast<long long>(s) * P + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, static_cast<long long>(p) * P + elem[q], wp[q]);
+                            load_state<UNIT>(a.w, static_cast<long long>(it.wp) * P + elem[q], wp[q]);
                             load_state<UNIT>(a.v, static_cast<long long>(p) * P + elem[q], vp[q]);
                         }
                     }
@@ -323,10 +345,10 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
                 for (int q = 0; q < U; ++q) {
                     if (live[q]) {
-                        load_state<UNIT>(a.w, static_cast<long long>(s) * P + elem[q], ws[q]);
+                        load_state<UNIT>(a.w, static_cast<long long>(it.ws) * P + elem[q], ws[q]);
                         load_state<UNIT>(a.v, static_cast<long long>(s) * P + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, static_cast<long long>(p) * P + elem[q], wp[q]);
+                            load_state<UNIT>(a.w, static_cast<long long>(it.wp) * P + elem[q], wp[q]);
                             load_state<UNIT>(a.v, static_cast<long long>(p) * P + elem[q], vp[q]);
                         }
                         sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, s, elem[q], gbs[q]);
@@ -367,13 +389,17 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     outs = us;
                 }
 
+                const long long wos = static_cast<long long>(it.wo_s) * P + elem[q];
                 store_state<UNIT>(a.v, os, vs[q]);
-                store_state<UNIT>(a.w, os, outs);
-                if constexpr (EMIT) store_bf16<UNIT>(a.wb, os, outs);
+                store_state<UNIT>(a.w, wos, outs);
+                if constexpr (EMIT) store_bf16<UNIT>(a.wb, wos, outs);
                 if constexpr (PAIRED) {
                     store_state<UNIT>(a.v, op, vp[q]);
-                    store_state<UNIT>(a.w, op, MODE == kPair ? outs : outp);
-                    if constexpr (EMIT) store_bf16<UNIT>(a.wb, op, MODE == kPair ? outs : outp);
+                    if (it.wo_p != it.wo_s) {      // pair members keep separate copies (block-uniform)
+                        const long long wop = static_cast<long long>(it.wo_p) * P + elem[q];
+                        store_state<UNIT>(a.w, wop, MODE == kPair ? outs : outp);
+                        if constexpr (EMIT) store_bf16<UNIT>(a.wb, wop, MODE == kPair ? outs : outp);
+                    }
                 }
 
                 if constexpr (DIAG) {
@@ -389,7 +415,17 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
         }
 
     }
-    if constexpr (DIAG) { if (cur >= 0) flush(cur); }
+
+    if constexpr (DIAG) {
+        if (cur >= 0) hand_over(cur);
+        // block partial of every item (zero for items this block never touched) -> partials[j][q][block]
+        __syncthreads();
+        for (int idx = tid; idx < a.n_work * kNQ; idx += THREADS) {
+            double tot = 0.;
+            for (int wi = 0; wi < WARPS; ++wi) tot += s_acc[static_cast<size_t>(wi) * a.n_work * kNQ + idx];  // fixed order
+            a.partials[static_cast<size_t>(idx) * gridDim.x + blockIdx.x] = tot;
+        }
+    }
 
     if constexpr (DIAG) {
         // last block to arrive reduces all block partials in a fixed order
@@ -409,7 +445,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                 sum = warp_sum(sum);
                 if (lane == 0) {
                     const int j = item / kNQ, k = item % kNQ;
-                    const int s = a.work[j].x, p = a.work[j].y;
+                    const Item it = unpack_item(a.work[j]);
+                    const int s = it.s, p = it.p;
                     // k: 0 gsq_s, 1 gsq_p, 2 wsq_s, 3 wsq_p, 4 gap (reported for both members)
                     double* gsq = a.diag; double* wsq = a.diag + a.S; double* gap = a.diag + 2 * a.S;
                     auto put = [&](double* dst, double val) { *dst = a.accumulate_diag ? *dst + val : val; };

@@ -189,6 +189,116 @@ def test_uniform_sweep_points(H, oracle_mod):
         assert_parity(gw, gv, ow, ov, True)
 
 
+# ------------------------------------------------------------------------------- shared pair storage
+
+@pytest.mark.parametrize("S,G,bf16", [(2, 2, False), (4, 4, False), (16, 4, False), (8, 8, True), (6, 3, False), (1, 2, False)])
+@pytest.mark.parametrize("exact", [True, False])
+def test_share_pair_weights_equals_oracle(H, oracle_mod, S, G, bf16, exact):
+    """HADPSGD_SHARE_PAIR_WEIGHTS: one weight buffer per pair, tile-major walk -- same arithmetic, so
+    the same bits as the oracle (ragged table, 5 steps = both parities, steady state reached)."""
+    flags = H.SHARE_PAIR_WEIGHTS | (H.DETERMINISTIC if exact else 0)
+    gw, gv, ow, ov = run_both(H, oracle_mod, S, G, ODD_TABLE, 5, bf16=bf16, flags=flags, seed=300 + S + G, v0_sd=0.01)
+    assert_parity(gw, gv, ow, ov, exact)
+
+
+def test_share_pair_weights_pointers_unshare_and_consensus(H, oracle_mod, torch_cuda):
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed = 8, 2, 100_003, 141
+    h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC | H.SHARE_PAIR_WEIGHTS, working_dtype=H.BF16)
+    problem.fill_weights(h, seed)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    ptr0 = [h.hadpsgd_weights(s).data_ptr() for s in range(S)]
+    assert len(set(ptr0)) == S                                     # before the first step: one buffer each
+    for k in range(3):
+        problem.fill_grads(h, seed, k)
+        h.hadpsgd_step(LR, MU, k)
+        oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k)
+        partner = H.hadpsgd_pairing(S, k)
+        ptr = [h.hadpsgd_weights(s).data_ptr() for s in range(S)]
+        assert all(ptr[s] == ptr[partner[s]] for s in range(S)) and len(set(ptr)) == S // 2
+        assert h.hadpsgd_consensus() == pytest.approx(oracle_mod.consensus_distance(ow), rel=1e-10)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    assert np.array_equal(bits(gw), bits(ow))
+    gb = np.stack([h.hadpsgd_weights_bf16(s).view(torch.int16)[:P].cpu().numpy().view(np.uint16) for s in range(S)])
+    assert np.array_equal(gb, oracle_mod.round_bf16(ow))
+    h.hadpsgd_unshare()                                            # every learner gets its own buffer back
+    ptr = [h.hadpsgd_weights(s).data_ptr() for s in range(S)]
+    assert len(set(ptr)) == S
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gb = np.stack([h.hadpsgd_weights_bf16(s).view(torch.int16)[:P].cpu().numpy().view(np.uint16) for s in range(S)])
+    assert np.array_equal(bits(gw), bits(ow)) and np.array_equal(gb, oracle_mod.round_bf16(ow))
+    h.hadpsgd_weights(3)[:P] += 1.0                                # now safe: nobody shares buffer 3
+    ow[3] += np.float32(1.0)
+    problem.fill_grads(h, seed, 3)
+    h.hadpsgd_step(LR, MU, 3)
+    oracle_mod.step(problem.host_grads(seed, 3, S, G, 0, P), ow, ov, LR, MU, 3)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    assert np.array_equal(bits(gw), bits(ow))
+    h.close()
+    for bad in (H.NO_MIX, H.EQ7_LITERAL):
+        with pytest.raises(H.HadpsgdError):
+            H.Hadpsgd(4, 2, [100], H.F32, H.SHARE_PAIR_WEIGHTS | bad)
+
+
+def test_share_pair_weights_with_custom_matchings_and_unpaired_members(H, oracle_mod, torch_cuda):
+    """Ring steps interleaved with caller-supplied matchings that leave members unmixed (odd S):
+    the shared buffers must be split again before an unmixed member updates in place."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed = 7, 2, 30_011, 151
+    matchings = [[1, 0, 3, 2, 5, 4, 6], [0, 2, 1, 4, 3, 6, 5], [6, 1, 2, 3, 4, 5, 0], [1, 0, 3, 2, 5, 4, 6],
+                 [0, 1, 2, 3, 4, 5, 6], [2, 3, 0, 1, 6, 5, 4]]
+    h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC | H.SHARE_PAIR_WEIGHTS)
+    problem.fill_weights(h, seed)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    for k, partner in enumerate(matchings):
+        problem.fill_grads(h, seed, k)
+        h.hadpsgd_step_matching(LR, MU, k, partner)
+        og = problem.host_grads(seed, k, S, G, 0, P)
+        groups = {tuple(sorted({s, partner[s]})) for s in range(S)}
+        for grp in groups:                                         # the step is pair-local: oracle per sub-ring
+            grp = list(grp)
+            w, v, g = ow[grp].copy(), ov[grp].copy(), np.ascontiguousarray(og[grp])
+            oracle_mod.step(g, w, v, LR, MU, 0)
+            ow[grp], ov[grp] = w, v
+        gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+        gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+        assert np.array_equal(bits(gw), bits(ow)) and np.array_equal(bits(gv), bits(ov)), k
+    h.close()
+
+
+def test_share_pair_weights_graph_replay_from_steady_state(H, oracle_mod, torch_cuda):
+    """With shared buffers the launch parameters depend on which buffer holds what; the pattern is
+    periodic with period 2 once one step has run, so an (odd, even) pair captured after one eager
+    step replays correctly."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed = 4, 2, 123_457, 161
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC | H.SHARE_PAIR_WEIGHTS, stream=side)
+        problem.fill_weights(h, seed)
+        problem.fill_grads(h, seed, 0)
+        h.hadpsgd_step(LR, MU, 0)                                  # eager: reaches the periodic state
+    side.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        h.hadpsgd_step(LR, MU, 1)
+        h.hadpsgd_step(LR, MU, 2)
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    og = problem.host_grads(seed, 0, S, G, 0, P)
+    for k in range(7):
+        oracle_mod.step(og, ow, ov, LR, MU, k)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    assert_parity(gw, gv, ow, ov, True)
+    h.close()
+
+
 # ------------------------------------------------------------------------------- API behaviour
 
 def test_custom_matching_and_unpaired(H, oracle_mod):
@@ -497,7 +607,7 @@ def windows_for(P, seg_len, n_win, width, seed):
     return wins[:n_win]
 
 
-def full_size_parity(H, oracle_mod, name, *, exact, n_win=6, width=8192):
+def full_size_parity(H, oracle_mod, name, *, exact, n_win=6, width=8192, extra_flags=0):
     """BASELINE.json full sizes, in the launch configuration bench.py times (default grid,
     diagnostics on): run all steps on the GPU with per-step regenerated gradients, then check
     sampled element windows against the oracle, which re-runs every step on each window with
@@ -509,7 +619,7 @@ def full_size_parity(H, oracle_mod, name, *, exact, n_win=6, width=8192):
     bf16 = cfg["grad"] == "bf16"
     seed = 1000 + len(name)
     P = int(sum(seg_len))
-    h = H.Hadpsgd(S, G, seg_len, H.BF16 if bf16 else H.F32, H.DETERMINISTIC if exact else 0)
+    h = H.Hadpsgd(S, G, seg_len, H.BF16 if bf16 else H.F32, (H.DETERMINISTIC if exact else 0) | extra_flags)
     problem.fill_weights(h, seed)
     diags = []
     for k in range(steps):
@@ -551,6 +661,14 @@ def test_config2_swb2000_full_size_exact(H, oracle_mod):
 
 def test_config2_swb2000_full_size_default_mode(H, oracle_mod):
     full_size_parity(H, oracle_mod, "swb2000", exact=False, n_win=4)
+
+
+def test_config2_and_3_full_size_shared_pair_weights(H, oracle_mod):
+    """The headline config and the ragged bf16 config with HADPSGD_SHARE_PAIR_WEIGHTS (the launch
+    configuration bench.py --flags share times)."""
+    full_size_parity(H, oracle_mod, "swb2000", exact=True, extra_flags=H.SHARE_PAIR_WEIGHTS)
+    full_size_parity(H, oracle_mod, "swb2000", exact=False, n_win=3, extra_flags=H.SHARE_PAIR_WEIGHTS)
+    full_size_parity(H, oracle_mod, "swb2000_ragged_bf16", exact=True, n_win=4, extra_flags=H.SHARE_PAIR_WEIGHTS)
 
 
 def test_config3_ragged_bf16_full_size(H, oracle_mod):
