@@ -35,6 +35,7 @@ FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the
 # `ncu --set full` capture summarised in profiles/ (bytes; None until a capture exists)
 NCU_TRAFFIC_BYTES = {"swb2000": 74.282e9, "swb300": 48.505e9, "swb2000_ragged_bf16": 37.124e9, "paper_literal": 16.537e9}
+NCU_TRAFFIC_SHARED = {"swb2000": 66.555e9, "swb2000_ragged_bf16": 33.285e9}     # same, with HADPSGD_SHARE_PAIR_WEIGHTS (profiles/r01_share_pair_weights.md)
 NCU_TRAFFIC_SOURCE = {"swb2000": "profiles/r01_step_kernel_ncu.md (dram__bytes_read.sum 55.737 GB + dram__bytes_write.sum 18.545 GB)",
                       "swb300": "profiles/r01_traffic_other_workloads.md", "swb2000_ragged_bf16": "profiles/r01_traffic_other_workloads.md",
                       "paper_literal": "profiles/r01_traffic_other_workloads.md"}
@@ -54,6 +55,7 @@ def parse_args():
     ap.add_argument("--cpu-sample-steps", type=int, default=20)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7,share")
+    ap.add_argument("--no-share-leg", action="store_true", help="skip the extra HADPSGD_SHARE_PAIR_WEIGHTS leg")
     ap.add_argument("--emit-bf16", action="store_true",
                     help="also write the bf16 working copy of the weights every step (row f2; +2 B/param)")
     ap.add_argument("--sweep", action="store_true",
@@ -397,7 +399,30 @@ def run_ours(args):
         if diag is not None:
             # the only collective: 3*S doubles, outside the timed region
             diag = sharding.allreduce_diagnostics(diag, dist, "cuda")
+    arena_bytes = h.arena_bytes
     h.close()
+    del h
+    torch.cuda.empty_cache()
+
+    # Second device-timed leg, reported beside the headline (never instead of it): the same step with
+    # HADPSGD_SHARE_PAIR_WEIGHTS, where pair members share one weight buffer (same arithmetic and
+    # results; one weight write per pair and one HBM fetch of the buffer two pairs read).
+    shared = None
+    can_share = not (flags & (H.NO_MIX | H.EQ7_LITERAL | H.SHARE_PAIR_WEIGHTS)) and S > 1 and S % 2 == 0
+    if can_share and not args.no_share_leg:
+        hs = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags | H.SHARE_PAIR_WEIGHTS,
+                       device=local, working_dtype=H.BF16 if args.emit_bf16 else H.F32)
+        problem.fill_weights(hs, seed)
+        problem.fill_grads(hs, seed, 0, cfg["dist"])
+        torch.cuda.synchronize()
+        s_secs, _ = time_device_steps(torch, dist, hs, args.steps, args.warmup)
+        if dist is not None:
+            from paper_1907_05701_b200 import sharding
+            s_secs = sharding.max_over_ranks(s_secs, dist, "cuda")
+        shared = s_secs / args.steps
+        hs.close()
+        del hs
+        torch.cuda.empty_cache()
 
     if rank == 0:
         t_step = secs / args.steps
@@ -411,7 +436,7 @@ def run_ours(args):
             "config": {"workload": args.workload, "S": S, "G": G, "P": P, "n_segments": len(cfg["seg_len"]),
                        "grad_dtype": cfg["grad"], "master_dtype": "f32",
                        "working_dtype": "bf16" if args.emit_bf16 else "f32", "lr": LR, "momentum": MU,
-                       "resident_bytes_per_gpu": h.arena_bytes, "flags": args.flags or "default (diagnostics on)",
+                       "resident_bytes_per_gpu": arena_bytes, "flags": args.flags or "default (diagnostics on)",
                        "l2": "inputs larger than L2 (working set per step >> 126 MB); no flush needed",
                        "parallelism": "single GPU" if world == 1 else f"parameter-range shards x{world}, no data-path collective"},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -421,6 +446,16 @@ def run_ours(args):
                          "kernel": "hadpsgd::step_kernel (one launch = one step)", "frac_of_8TBps_nominal": achieved / 8000.0},
             "clocks": clocks, "gpu_launches": launches,
         }
+        if shared is not None:
+            line["share_pair_weights"] = {
+                "flag": "HADPSGD_SHARE_PAIR_WEIGHTS (opt-in; bench.py --flags share makes it the headline leg)",
+                "ms_per_step": shared * 1e3, "value": world * S * G * P / shared, "unit": UNIT,
+                "achieved_algorithmic_gbs": abytes / shared / 1e9, "frac_of_peak_algorithmic": abytes / shared / 1e9 / peak,
+                "bytes_moved_model": S * P * (cfg["G"] * cfg["b_g"] + 12 + (1 if args.emit_bf16 else 0)),
+                "traffic": NCU_TRAFFIC_SHARED.get(args.workload) if not args.emit_bf16 else None,
+                "note": "same arithmetic and results (parity-tested at full size); pair members share one of the S weight "
+                        "buffers: 4 B less written and 4 B less fetched from HBM per pair-parameter than the algorithmic "
+                        "S*P*(G*b_g+16), so achieved_algorithmic_gbs exceeds the DRAM rate actually sustained"}
         if e2e:
             e_step = e2e[0] / args.e2e_steps
             line["e2e"] = {"value": world * S * G * P / e_step, "unit": UNIT, "h2d_bytes_per_step": e2e[1],

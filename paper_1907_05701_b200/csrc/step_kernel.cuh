@@ -116,11 +116,10 @@ __device__ __forceinline__ void widen(const Raw8& raw, Vec<UNIT>& out) {
 
 // Issue the G learner-gradient loads of super-learner s for one unit (a2); raw registers.
 template <int G, bool BF16>
-__device__ __forceinline__ void load_grads(const char* gbase, long long P, int s, long long elem, Raw8 (&gr)[G]) {
-    constexpr int EB = BF16 ? 2 : 4;
+__device__ __forceinline__ void load_grads(const char* gbase, long long P, long long off0, Raw8 (&gr)[G]) {
+    constexpr int EB = BF16 ? 2 : 4;   // off0 = element offset inside learner 0's buffer of this super-learner
 #pragma unroll
-    for (int k = 0; k < G; ++k)
-        gr[k] = ld_stream32(gbase + ((static_cast<long long>(s) * G + k) * P + elem) * EB);
+    for (int k = 0; k < G; ++k) gr[k] = ld_stream32(gbase + (off0 + k * P) * EB);
 }
 
 template <int UNIT>
@@ -180,10 +179,10 @@ __device__ __forceinline__ void sum_grads(const Raw8 (&gr)[G], Vec<UNIT>& acc) {
 
 // Runtime-G sum (any G >= 1): learners are streamed in batches of 4 loads, left to right.
 template <bool BF16, bool EXACT, int UNIT>
-__device__ __forceinline__ void sum_grads_runtime(const char* gbase, long long P, int G, int s, long long elem,
+__device__ __forceinline__ void sum_grads_runtime(const char* gbase, long long P, int G, long long off0,
                                                   Vec<UNIT>& acc) {
     constexpr int EB = BF16 ? 2 : 4;
-    const char* p0 = gbase + (static_cast<long long>(s) * G * P + elem) * EB;
+    const char* p0 = gbase + off0 * EB;
     const long long stride = P * EB;
     widen<BF16, UNIT>(ld_stream32(p0), acc);
     int k = 1;
@@ -283,6 +282,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     double d_gs = 0., d_gp = 0., d_ws = 0., d_wp = 0., d_gap = 0.;
     int cur = -1;
     Item it = {0, 0, 0, 0, 0, 0};
+    // element offsets of the current item's buffers, recomputed only when the item changes
+    long long o_vs = 0, o_vp = 0, o_ws = 0, o_wp = 0, o_wos = 0, o_wop = 0, o_gs = 0, o_gp = 0;
     auto hand_over = [&](int item) {
         if constexpr (MODE == kPair) d_wp = d_ws;
         double q[kNQ] = {d_gs, d_gp, d_ws, d_wp, d_gap};
@@ -305,8 +306,11 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             if constexpr (DIAG) { if (cur >= 0) hand_over(cur); }
             cur = j;
             it = unpack_item(a.work[j]);
+            o_vs = it.s * P; o_vp = it.p * P;                   // momentum: the member's own buffer
+            o_ws = it.ws * P; o_wp = it.wp * P;                 // weights are read from these slots ...
+            o_wos = it.wo_s * P; o_wop = it.wo_p * P;           // ... and written to these
+            o_gs = o_vs * a.G; o_gp = o_vp * a.G;               // learner 0 of each member
         }
-        const int s = it.s, p = it.p;
         {
             Vec<UNIT> ws[U], vs[U], gbs[U], wp[NP], vp[NP], gbp[NP];
             bool live[U];
@@ -324,13 +328,13 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
                 for (int q = 0; q < U; ++q) {
                     if (live[q]) {
-                        load_grads<GA, BF16>(gbytes, P, s, elem[q], grs[q]);
-                        if constexpr (PAIRED) load_grads<GA, BF16>(gbytes, P, p, elem[q], grp[q]);
-                        load_state<UNIT>(a.w, static_cast<long long>(it.ws) * P + elem[q], ws[q]);
-                        load_state<UNIT>(a.v, static_cast<long long>(s) * P + elem[q], vs[q]);
+                        load_grads<GA, BF16>(gbytes, P, o_gs + elem[q], grs[q]);
+                        if constexpr (PAIRED) load_grads<GA, BF16>(gbytes, P, o_gp + elem[q], grp[q]);
+                        load_state<UNIT>(a.w, o_ws + elem[q], ws[q]);
+                        load_state<UNIT>(a.v, o_vs + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, static_cast<long long>(it.wp) * P + elem[q], wp[q]);
-                            load_state<UNIT>(a.v, static_cast<long long>(p) * P + elem[q], vp[q]);
+                            load_state<UNIT>(a.w, o_wp + elem[q], wp[q]);
+                            load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
                     }
                 }
@@ -345,14 +349,14 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
                 for (int q = 0; q < U; ++q) {
                     if (live[q]) {
-                        load_state<UNIT>(a.w, static_cast<long long>(it.ws) * P + elem[q], ws[q]);
-                        load_state<UNIT>(a.v, static_cast<long long>(s) * P + elem[q], vs[q]);
+                        load_state<UNIT>(a.w, o_ws + elem[q], ws[q]);
+                        load_state<UNIT>(a.v, o_vs + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, static_cast<long long>(it.wp) * P + elem[q], wp[q]);
-                            load_state<UNIT>(a.v, static_cast<long long>(p) * P + elem[q], vp[q]);
+                            load_state<UNIT>(a.w, o_wp + elem[q], wp[q]);
+                            load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
-                        sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, s, elem[q], gbs[q]);
-                        if constexpr (PAIRED) sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, p, elem[q], gbp[q]);
+                        sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, o_gs + elem[q], gbs[q]);
+                        if constexpr (PAIRED) sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, o_gp + elem[q], gbp[q]);
                     }
                 }
             }
@@ -360,8 +364,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
             for (int q = 0; q < U; ++q) {
                 if (!live[q]) continue;
-                const long long os = static_cast<long long>(s) * P + elem[q];
-                const long long op = static_cast<long long>(p) * P + elem[q];
+                const long long os = o_vs + elem[q];
+                const long long op = o_vp + elem[q];
                 Vec<UNIT> us, up, outs, outp, dif;
                 apply_update<EXACT, UNIT>(gbs[q], invG, mu, lr, ws[q], vs[q], us);
                 if constexpr (PAIRED) apply_update<EXACT, UNIT>(gbp[q], invG, mu, lr, wp[q], vp[q], up);
@@ -389,14 +393,14 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     outs = us;
                 }
 
-                const long long wos = static_cast<long long>(it.wo_s) * P + elem[q];
+                const long long wos = o_wos + elem[q];
                 store_state<UNIT>(a.v, os, vs[q]);
                 store_state<UNIT>(a.w, wos, outs);
                 if constexpr (EMIT) store_bf16<UNIT>(a.wb, wos, outs);
                 if constexpr (PAIRED) {
                     store_state<UNIT>(a.v, op, vp[q]);
                     if (it.wo_p != it.wo_s) {      // pair members keep separate copies (block-uniform)
-                        const long long wop = static_cast<long long>(it.wo_p) * P + elem[q];
+                        const long long wop = o_wop + elem[q];
                         store_state<UNIT>(a.w, wop, MODE == kPair ? outs : outp);
                         if constexpr (EMIT) store_bf16<UNIT>(a.wb, wop, MODE == kPair ? outs : outp);
                     }
