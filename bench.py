@@ -34,7 +34,7 @@ LR, MU = 0.1, 0.9
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the
 # `ncu --set full` capture summarised in profiles/ (bytes; None until a capture exists)
-NCU_TRAFFIC_BYTES = {"swb2000": 74.282e9, "swb300": 48.505e9, "swb2000_ragged_bf16": 37.124e9, "paper_literal": 16.537e9}
+NCU_TRAFFIC_BYTES = {"swb2000": 74.284e9, "swb300": 48.502e9, "swb2000_ragged_bf16": 37.123e9, "paper_literal": 16.536e9}
 NCU_TRAFFIC_SHARED = {"swb2000": 66.555e9, "swb2000_ragged_bf16": 33.285e9}     # same, with HADPSGD_SHARE_PAIR_WEIGHTS (profiles/r01_share_pair_weights.md)
 NCU_TRAFFIC_SOURCE = {"swb2000": "profiles/r01_step_kernel_ncu.md (dram__bytes_read.sum 55.737 GB + dram__bytes_write.sum 18.545 GB)",
                       "swb300": "profiles/r01_traffic_other_workloads.md", "swb2000_ragged_bf16": "profiles/r01_traffic_other_workloads.md",
