@@ -328,16 +328,17 @@ def test_custom_matching_and_unpaired(H, oracle_mod):
     h.close()
 
 
-def test_host_gradient_path_equals_resident_path(H, oracle_mod):
+@pytest.mark.parametrize("share", [False, True])
+def test_host_gradient_path_equals_resident_path(H, oracle_mod, share):
     """hadpsgd_step_host (the e2e entry): chunked H2D + kernel on element sub-ranges must give
     the same bits and the same diagnostics as the resident-gradient step.  P spans 3 chunks."""
     import torch
     from fixtures import problem
-    S, G, seed = 2, 2, 91
+    S, G, seed = 4, 2, 91
     P = (8 << 20) * 2 + 12_345 * 64
     outs = []
     for path in ("resident", "host"):
-        h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
+        h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC | (H.SHARE_PAIR_WEIGHTS if share else 0))
         problem.fill_weights(h, seed)
         for k in range(2):
             problem.fill_grads(h, seed, k)
