@@ -63,14 +63,15 @@ struct DeviceGuard {
     DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
-int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, bool tile_major, float lr, float mu,
+int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, bool shared_slots, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
     const bool exact = h->flags & HADPSGD_DETERMINISTIC;
     const bool diag = !(h->flags & HADPSGD_NO_DIAG);
     const bool emit = h->L.working_dtype == HADPSGD_BF16;
-    LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode) : plan_f32_emit(h->L.G, exact, diag, mode))
-                           : (bf16 ? plan_bf16(h->L.G, exact, diag, mode) : plan_f32(h->L.G, exact, diag, mode));
+    const bool shared = shared_slots && mode == kPair;   // pair members share weight slots
+    LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode, shared) : plan_f32_emit(h->L.G, exact, diag, mode, shared))
+                           : (bf16 ? plan_bf16(h->L.G, exact, diag, mode, shared) : plan_f32(h->L.G, exact, diag, mode, shared));
 
     const int unit = bf16 ? 16 : 8;   // elements per 32-byte gradient vector
     StepArgs a;
@@ -88,7 +89,6 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
     a.accumulate_diag = accumulate ? 1 : 0;
     a.S = h->L.S;
     a.partials = h->d_partials; a.diag = h->d_diag; a.ticket = h->d_ticket;
-    a.tile_major = tile_major ? 1 : 0;
     for (int j = 0; j < n_items; ++j)
         a.work[j] = pack_item(items[j].s, items[j].p, items[j].ws, items[j].wp, items[j].wo_s, items[j].wo_p);
 
@@ -126,12 +126,12 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
 
 // All items of one mode over [elem_begin, elem_end); more than kMaxWork items (S > 480 unmixed
 // super-learners) take several launches.
-int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, bool tile_major, float lr, float mu,
+int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, bool shared_slots, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     if (elem_end <= elem_begin) return HADPSGD_OK;
     for (size_t first = 0; first < items.size(); first += kMaxWork) {
         const int n = static_cast<int>(items.size() - first < static_cast<size_t>(kMaxWork) ? items.size() - first : kMaxWork);
-        int rc = launch_chunk(h, items.data() + first, n, mode, tile_major, lr, mu, elem_begin, elem_end, accumulate);
+        int rc = launch_chunk(h, items.data() + first, n, mode, shared_slots, lr, mu, elem_begin, elem_end, accumulate);
         if (rc != HADPSGD_OK) return rc;
     }
     return HADPSGD_OK;

@@ -46,7 +46,6 @@ struct StepArgs {
     double* partials;     // [n_work][kNQ][gridDim.x]
     double* diag;         // gsq[S] | wsq[S] | gap[S]
     unsigned int* ticket;
-    int tile_major;       // 0: item-major tile walk; 1: tile-major (all items of a tile, then the next)
     unsigned long long work[kMaxWork];   // six 10-bit fields per item, see pack_item()
 };
 
@@ -245,11 +244,16 @@ __device__ __forceinline__ double warp_sum(double x) {
 // THREADS x U units; thread t owns units t, t+THREADS, ... of the tile, so each warp request
 // covers 1 KB contiguous of one stream.
 // ---------------------------------------------------------------------------------------
-template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, bool EMIT, int U, int THREADS, int MINB>
+// SHARED (kPair only): pair members share weight slots (HADPSGD_SHARE_PAIR_WEIGHTS): weights are
+// read from the item's read slots, the mixed weights are stored ONCE, and the walk is tile-major.
+template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, bool EMIT, bool SHARED, int U, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_constant__ StepArgs a) {
     constexpr int UNIT = BF16 ? 16 : 8;
     constexpr int GA = G > 0 ? G : 1;
     constexpr bool PAIRED = (MODE != kSingle);
+    // weights addressed through the item's slots: shared pairs, and every unmixed item (after an
+    // un-sharing copy the slot of an unmixed member need not be its own index)
+    constexpr bool SLOTS = SHARED || MODE == kSingle;
     constexpr int NP = PAIRED ? U : 1;   // array extent of the partner's registers
     constexpr int WARPS = THREADS / 32;
     extern __shared__ double s_acc[];    // DIAG: [WARPS][n_work][kNQ], each warp owns its rows
@@ -283,7 +287,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     int cur = -1;
     Item it = {0, 0, 0, 0, 0, 0};
     // element offsets of the current item's buffers, recomputed only when the item changes
-    long long o_vs = 0, o_vp = 0, o_ws = 0, o_wp = 0, o_wos = 0, o_wop = 0, o_gs = 0, o_gp = 0;
+    long long o_vs = 0, o_vp = 0, o_gs = 0, o_gp = 0;   // momentum / gradients: the member's own buffers
+    long long o_ws = 0, o_wp = 0, o_wo = 0;             // SHARED: weight read slots and the one write slot
     auto hand_over = [&](int item) {
         if constexpr (MODE == kPair) d_wp = d_ws;
         double q[kNQ] = {d_gs, d_gp, d_ws, d_wp, d_gap};
@@ -299,17 +304,16 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     for (long long gt = blockIdx.x; gt < total_tiles; gt += gridDim.x) {
         int j;
         long long tile;
-        if (a.tile_major) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
+        if constexpr (SHARED) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
         else { j = static_cast<int>(gt / n_tiles); tile = gt - static_cast<long long>(j) * n_tiles; }
         const long long base = tile * TILE;
         if (j != cur) {                                  // block-uniform
             if constexpr (DIAG) { if (cur >= 0) hand_over(cur); }
             cur = j;
             it = unpack_item(a.work[j]);
-            o_vs = it.s * P; o_vp = it.p * P;                   // momentum: the member's own buffer
-            o_ws = it.ws * P; o_wp = it.wp * P;                 // weights are read from these slots ...
-            o_wos = it.wo_s * P; o_wop = it.wo_p * P;           // ... and written to these
+            o_vs = it.s * P; o_vp = it.p * P;
             o_gs = o_vs * a.G; o_gp = o_vp * a.G;               // learner 0 of each member
+            if constexpr (SLOTS) { o_ws = it.ws * P; o_wp = it.wp * P; o_wo = it.wo_s * P; }
         }
         {
             Vec<UNIT> ws[U], vs[U], gbs[U], wp[NP], vp[NP], gbp[NP];
@@ -330,10 +334,10 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     if (live[q]) {
                         load_grads<GA, BF16>(gbytes, P, o_gs + elem[q], grs[q]);
                         if constexpr (PAIRED) load_grads<GA, BF16>(gbytes, P, o_gp + elem[q], grp[q]);
-                        load_state<UNIT>(a.w, o_ws + elem[q], ws[q]);
+                        load_state<UNIT>(a.w, (SLOTS ? o_ws : o_vs) + elem[q], ws[q]);
                         load_state<UNIT>(a.v, o_vs + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, o_wp + elem[q], wp[q]);
+                            load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
                             load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
                     }
@@ -349,10 +353,10 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
                 for (int q = 0; q < U; ++q) {
                     if (live[q]) {
-                        load_state<UNIT>(a.w, o_ws + elem[q], ws[q]);
+                        load_state<UNIT>(a.w, (SLOTS ? o_ws : o_vs) + elem[q], ws[q]);
                         load_state<UNIT>(a.v, o_vs + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, o_wp + elem[q], wp[q]);
+                            load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
                             load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
                         sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, o_gs + elem[q], gbs[q]);
@@ -393,16 +397,15 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     outs = us;
                 }
 
-                const long long wos = o_wos + elem[q];
+                const long long wos = SLOTS ? o_wo + elem[q] : os;
                 store_state<UNIT>(a.v, os, vs[q]);
                 store_state<UNIT>(a.w, wos, outs);
                 if constexpr (EMIT) store_bf16<UNIT>(a.wb, wos, outs);
                 if constexpr (PAIRED) {
                     store_state<UNIT>(a.v, op, vp[q]);
-                    if (it.wo_p != it.wo_s) {      // pair members keep separate copies (block-uniform)
-                        const long long wop = o_wop + elem[q];
-                        store_state<UNIT>(a.w, wop, MODE == kPair ? outs : outp);
-                        if constexpr (EMIT) store_bf16<UNIT>(a.wb, wop, MODE == kPair ? outs : outp);
+                    if constexpr (!SHARED) {       // pair members keep separate copies
+                        store_state<UNIT>(a.w, op, MODE == kPair ? outs : outp);
+                        if constexpr (EMIT) store_bf16<UNIT>(a.wb, op, MODE == kPair ? outs : outp);
                     }
                 }
 
