@@ -32,11 +32,15 @@ def lib():
         L.hadpsgd_oracle_mixing_matrix.argtypes = [i32, u64, vp]
         L.hadpsgd_oracle_step.argtypes = [i32, i32, i64, vp, i32, vp, vp, f32, f32, u64, u32, vp]
         L.hadpsgd_oracle_step_f64.argtypes = [i32, i32, i64, vp, i32, vp, vp, f64, f64, u64, u32]
+        L.hadpsgd_oracle_step_matching.argtypes = [i32, i32, i64, vp, i32, vp, vp, f32, f32, vp, u32, vp]
+        L.hadpsgd_oracle_step_matching_f64.argtypes = [i32, i32, i64, vp, i32, vp, vp, f64, f64, vp, u32]
+        L.hadpsgd_oracle_mixing_matrix_matching.argtypes = [i32, vp, vp]
         L.hadpsgd_oracle_consensus_distance.argtypes = [i32, i64, vp, vp]
         L.hadpsgd_oracle_round_bf16.argtypes = [i64, vp, vp]
         L.hadpsgd_oracle_round_bf16.restype = i32
         for fn in (L.hadpsgd_oracle_partner, L.hadpsgd_oracle_mixing_matrix, L.hadpsgd_oracle_step,
-                   L.hadpsgd_oracle_step_f64, L.hadpsgd_oracle_consensus_distance):
+                   L.hadpsgd_oracle_step_f64, L.hadpsgd_oracle_consensus_distance, L.hadpsgd_oracle_step_matching,
+                   L.hadpsgd_oracle_step_matching_f64, L.hadpsgd_oracle_mixing_matrix_matching):
             fn.restype = i32
         _lib = L
     return _lib
@@ -76,15 +80,39 @@ def _check(grads, w, v, wdtype):
     return S, G, P, gd
 
 
-def step(grads, w, v, lr, mu, step_k, flags=0, diag=False):
+def _matching(partner, S):
+    p = np.ascontiguousarray(partner, dtype=np.int32)
+    if p.shape != (S,):
+        raise ValueError("partner must have S entries")
+    return p
+
+
+def mixing_matrix_matching(partner):
+    p = _matching(partner, len(partner))
+    T = np.empty((len(p), len(p)), dtype=np.float64)
+    rc = lib().hadpsgd_oracle_mixing_matrix_matching(len(p), _ptr(p), _ptr(T))
+    if rc != 0:
+        raise ValueError("hadpsgd_oracle_mixing_matrix_matching: partner is not a matching")
+    return T
+
+
+def step(grads, w, v, lr, mu, step_k, flags=0, diag=False, partner=None):
     """In-place fp32 step on w, v (numpy float32 [S,P]); grads [S,G,P] float32 or uint16(bf16).
+    partner=None: the ring matching of step_k's parity; else a caller-supplied matching [S]
+    (an involution; partner[s] == s leaves s unmixed).
 
     Returns None, or a dict of double arrays gsq[S], wsq[S], gap[S] when diag=True."""
     S, G, P, gd = _check(grads, w, v, np.float32)
     d = np.zeros(3 * S, dtype=np.float64) if diag else None
-    rc = lib().hadpsgd_oracle_step(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
-                                   float(lr), float(mu), int(step_k), int(flags),
-                                   _ptr(d) if diag else None)
+    if partner is None:
+        rc = lib().hadpsgd_oracle_step(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
+                                       float(lr), float(mu), int(step_k), int(flags),
+                                       _ptr(d) if diag else None)
+    else:
+        pt = _matching(partner, S)
+        rc = lib().hadpsgd_oracle_step_matching(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
+                                                float(lr), float(mu), _ptr(pt), int(flags),
+                                                _ptr(d) if diag else None)
     if rc != 0:
         raise ValueError(f"hadpsgd_oracle_step rc={rc}")
     if diag:
@@ -92,11 +120,16 @@ def step(grads, w, v, lr, mu, step_k, flags=0, diag=False):
     return None
 
 
-def step_f64(grads, w, v, lr, mu, step_k, flags=0):
+def step_f64(grads, w, v, lr, mu, step_k, flags=0, partner=None):
     """In-place double-precision shadow step on w, v (numpy float64 [S,P])."""
     S, G, P, gd = _check(grads, w, v, np.float64)
-    rc = lib().hadpsgd_oracle_step_f64(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
-                                       float(lr), float(mu), int(step_k), int(flags))
+    if partner is None:
+        rc = lib().hadpsgd_oracle_step_f64(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
+                                           float(lr), float(mu), int(step_k), int(flags))
+    else:
+        pt = _matching(partner, S)
+        rc = lib().hadpsgd_oracle_step_matching_f64(S, G, P, _ptr(grads), gd, _ptr(w), _ptr(v),
+                                                    float(lr), float(mu), _ptr(pt), int(flags))
     if rc != 0:
         raise ValueError(f"hadpsgd_oracle_step_f64 rc={rc}")
 

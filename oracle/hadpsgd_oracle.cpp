@@ -51,6 +51,30 @@ bool build_partner(int S, uint64_t step_k, uint32_t flags, std::vector<int32_t>&
     return true;
 }
 
+// A caller-supplied matching (R8): an involution on {0..S-1}; partner[s] == s
+// leaves s unmixed (row and column s of T_k hold a single 1).
+bool copy_matching(int S, const int32_t* in, std::vector<int32_t>& partner) {
+    if (S < 1 || !in) return false;
+    partner.assign(in, in + S);
+    for (int s = 0; s < S; ++s) {
+        int p = partner[s];
+        if (p < 0 || p >= S || partner[p] != s) return false;
+    }
+    return true;
+}
+
+void dense_T(int S, const std::vector<int32_t>& p, double* T) {
+    for (int64_t k = 0; k < static_cast<int64_t>(S) * S; ++k) T[k] = 0.0;
+    for (int s = 0; s < S; ++s) {
+        if (p[s] == s) {
+            T[static_cast<int64_t>(s) * S + s] = 1.0;
+        } else {
+            T[static_cast<int64_t>(s) * S + s] = 0.5;
+            T[static_cast<int64_t>(s) * S + p[s]] = 0.5;
+        }
+    }
+}
+
 }  // namespace
 
 extern "C" int hadpsgd_oracle_partner(int S, uint64_t step_k, int32_t* partner) {
@@ -65,26 +89,23 @@ extern "C" int hadpsgd_oracle_mixing_matrix(int S, uint64_t step_k, double* T) {
     if (!T) return -1;
     std::vector<int32_t> p;
     if (!build_partner(S, step_k, 0, p)) return -1;
-    for (int64_t k = 0; k < static_cast<int64_t>(S) * S; ++k) T[k] = 0.0;
-    for (int s = 0; s < S; ++s) {
-        if (p[s] == s) {
-            T[static_cast<int64_t>(s) * S + s] = 1.0;
-        } else {
-            T[static_cast<int64_t>(s) * S + s] = 0.5;
-            T[static_cast<int64_t>(s) * S + p[s]] = 0.5;
-        }
-    }
+    dense_T(S, p, T);
     return 0;
 }
 
-extern "C" int hadpsgd_oracle_step(int S, int G, int64_t P, const void* grads, int grad_dtype,
-                                   float* w, float* v, float lr, float mu, uint64_t step_k,
-                                   uint32_t flags, double* diag) {
-    if (S < 1 || G < 1 || P < 0 || !grads || !w || !v) return -1;
-    if (grad_dtype != ORACLE_GRAD_F32 && grad_dtype != ORACLE_GRAD_BF16) return -1;
-    std::vector<int32_t> partner;
-    if (!build_partner(S, step_k, flags, partner)) return -1;
+extern "C" int hadpsgd_oracle_mixing_matrix_matching(int S, const int32_t* partner, double* T) {
+    if (!T) return -1;
+    std::vector<int32_t> p;
+    if (!copy_matching(S, partner, p)) return -1;
+    dense_T(S, p, T);
+    return 0;
+}
 
+namespace {
+
+// The step for a given matching `partner` (ring or caller-supplied).
+int step_f32(int S, int G, int64_t P, const void* grads, int grad_dtype, float* w, float* v,
+             float lr, float mu, const std::vector<int32_t>& partner, uint32_t flags, double* diag) {
     const float invG = 1.0f / static_cast<float>(G);  // R5: mean = fp32 sum * fp32 reciprocal
     std::vector<float> u(static_cast<size_t>(S) * static_cast<size_t>(P));
     double* gsq = diag ? diag : nullptr;
@@ -112,13 +133,18 @@ extern "C" int hadpsgd_oracle_step(int S, int G, int64_t P, const void* grads, i
         }
     }
 
-    // phase 2: pairwise averaging with the ring neighbour (eq. (7), T_k)
+    // phase 2: pairwise averaging with the matched neighbour (eq. (7), T_k).
+    // Diagnostics (R14): gap[s] = sum_i (a_s - a_p)^2 over the two vectors the mix
+    // AVERAGES -- u_s, u_p by default; the OLD weights w_s, w_p under EQ7_LITERAL (PAPER.md:64
+    // mixes Theta_k itself) -- so an unpaired member (p == s) has gap exactly 0.  wsq[s] is
+    // always the sum of squares of the weights s holds AFTER the step.
     for (int s = 0; s < S; ++s) {
         int p = partner[s];
         if (p < s) continue;  // each pair once; p == s means unpaired
         for (int64_t i = 0; i < P; ++i) {
             if (flags & ORACLE_EQ7_LITERAL) {
-                // Theta_{k+1} = Theta_k T_k - alpha g : mix OLD weights, subtract own update
+                // Theta_{k+1} = Theta_k T_k - alpha g : mix OLD weights, subtract own update.
+                // fp32 order (R14): m = 0.5f*(w_s + w_p); t = lr*v' (phase 1); w' = m - t.
                 float ws = w[s * P + i], wp = w[p * P + i];
                 float m = (p == s) ? ws : 0.5f * (ws + wp);
                 if (diag) {
@@ -148,14 +174,8 @@ extern "C" int hadpsgd_oracle_step(int S, int G, int64_t P, const void* grads, i
     return 0;
 }
 
-extern "C" int hadpsgd_oracle_step_f64(int S, int G, int64_t P, const void* grads, int grad_dtype,
-                                       double* w, double* v, double lr, double mu,
-                                       uint64_t step_k, uint32_t flags) {
-    if (S < 1 || G < 1 || P < 0 || !grads || !w || !v) return -1;
-    if (grad_dtype != ORACLE_GRAD_F32 && grad_dtype != ORACLE_GRAD_BF16) return -1;
-    std::vector<int32_t> partner;
-    if (!build_partner(S, step_k, flags, partner)) return -1;
-
+int step_f64(int S, int G, int64_t P, const void* grads, int grad_dtype, double* w, double* v,
+             double lr, double mu, const std::vector<int32_t>& partner, uint32_t flags) {
     std::vector<double> u(static_cast<size_t>(S) * static_cast<size_t>(P));
     for (int s = 0; s < S; ++s) {
         for (int64_t i = 0; i < P; ++i) {
@@ -188,6 +208,51 @@ extern "C" int hadpsgd_oracle_step_f64(int S, int G, int64_t P, const void* grad
         }
     }
     return 0;
+}
+
+bool args_ok(int S, int G, int64_t P, const void* grads, int grad_dtype, const void* w, const void* v) {
+    if (S < 1 || G < 1 || P < 0 || !grads || !w || !v) return false;
+    return grad_dtype == ORACLE_GRAD_F32 || grad_dtype == ORACLE_GRAD_BF16;
+}
+
+}  // namespace
+
+// Ring schedule (north_star (b), R7): the matching comes from step_k's parity.
+extern "C" int hadpsgd_oracle_step(int S, int G, int64_t P, const void* grads, int grad_dtype,
+                                   float* w, float* v, float lr, float mu, uint64_t step_k,
+                                   uint32_t flags, double* diag) {
+    if (!args_ok(S, G, P, grads, grad_dtype, w, v)) return -1;
+    std::vector<int32_t> partner;
+    if (!build_partner(S, step_k, flags, partner)) return -1;
+    return step_f32(S, G, P, grads, grad_dtype, w, v, lr, mu, partner, flags, diag);
+}
+
+extern "C" int hadpsgd_oracle_step_f64(int S, int G, int64_t P, const void* grads, int grad_dtype,
+                                       double* w, double* v, double lr, double mu,
+                                       uint64_t step_k, uint32_t flags) {
+    if (!args_ok(S, G, P, grads, grad_dtype, w, v)) return -1;
+    std::vector<int32_t> partner;
+    if (!build_partner(S, step_k, flags, partner)) return -1;
+    return step_f64(S, G, P, grads, grad_dtype, w, v, lr, mu, partner, flags);
+}
+
+// Caller-supplied matching (row f1, R8): any involution, unpaired members allowed (T_ss = 1).
+extern "C" int hadpsgd_oracle_step_matching(int S, int G, int64_t P, const void* grads, int grad_dtype,
+                                            float* w, float* v, float lr, float mu,
+                                            const int32_t* partner_in, uint32_t flags, double* diag) {
+    if (!args_ok(S, G, P, grads, grad_dtype, w, v)) return -1;
+    std::vector<int32_t> partner;
+    if (!copy_matching(S, partner_in, partner)) return -1;
+    return step_f32(S, G, P, grads, grad_dtype, w, v, lr, mu, partner, flags, diag);
+}
+
+extern "C" int hadpsgd_oracle_step_matching_f64(int S, int G, int64_t P, const void* grads, int grad_dtype,
+                                                double* w, double* v, double lr, double mu,
+                                                const int32_t* partner_in, uint32_t flags) {
+    if (!args_ok(S, G, P, grads, grad_dtype, w, v)) return -1;
+    std::vector<int32_t> partner;
+    if (!copy_matching(S, partner_in, partner)) return -1;
+    return step_f64(S, G, P, grads, grad_dtype, w, v, lr, mu, partner, flags);
 }
 
 extern "C" int hadpsgd_oracle_round_bf16(int64_t n, const float* w, uint16_t* out) {

@@ -55,16 +55,37 @@ int hadpsgd_oracle_mixing_matrix(int S, uint64_t step_k, double* T /*[S*S]*/);
  *       u    = w - lr*v             (mul, then sub)
  *   phase 2 (eq. (7), T_k PAPER.md:66, order per PAPER.md:62, R3):
  *       w_s = w_p = 0.5f * (u_s + u_p)
- * diag (optional, may be NULL): doubles laid out
- *       gsq[S] | wsq[S] | gap[S]   (gap[s] == gap[partner[s]]; 0 if unpaired)
- *   gsq[s] = sum_i gbar^2, wsq[s] = sum_i w'^2, gap[s] = sum_i (u_s-u_p)^2,
- *   each term formed in double from the fp32 values.
+ *   with ORACLE_EQ7_LITERAL (eq. (7) as printed; fp32 order fixed by R14):
+ *       m = 0.5f * (w_s + w_p)  (OLD weights) ;  t_s = lr * v_s  (the new v) ;  w_s = m - t_s
+ * diag (optional, may be NULL): doubles laid out  (R14)
+ *       gsq[S] | wsq[S] | gap[S]   (gap[s] == gap[partner[s]]; exactly 0 if unpaired)
+ *   gsq[s] = sum_i gbar^2, wsq[s] = sum_i w'_s^2 (the weights s holds after the step),
+ *   gap[s] = sum_i (a_s-a_p)^2 over the two vectors the mix averages: a = u by default,
+ *   a = the OLD weights w under ORACLE_EQ7_LITERAL; each term formed in double from the
+ *   fp32 values.
  * grads are read-only; w and v are updated in place.                          */
 int hadpsgd_oracle_step(int S, int G, int64_t P,
                         const void* grads, int grad_dtype,
                         float* w, float* v,
                         float lr, float mu, uint64_t step_k, uint32_t flags,
                         double* diag /* [3*S] or NULL */);
+
+/* The same step for a CALLER-SUPPLIED matching (R8): partner
+ * [S] must be an involution (partner[partner[s]] == s, else -1); partner[s] == s leaves s
+ * unmixed, i.e. row and column s of T_k hold a single 1 (PAPER.md:66 generalised: T_k stays
+ * symmetric and doubly stochastic).  Odd S is fine.  ORACLE_NO_MIX is ignored here (pass the
+ * identity instead).  Diagnostics as above; gap[s] == 0 exactly for an unmixed member.       */
+int hadpsgd_oracle_step_matching(int S, int G, int64_t P,
+                                 const void* grads, int grad_dtype,
+                                 float* w, float* v,
+                                 float lr, float mu, const int32_t* partner /*[S]*/, uint32_t flags,
+                                 double* diag /* [3*S] or NULL */);
+int hadpsgd_oracle_step_matching_f64(int S, int G, int64_t P,
+                                     const void* grads, int grad_dtype,
+                                     double* w, double* v,
+                                     double lr, double mu, const int32_t* partner /*[S]*/, uint32_t flags);
+/* Dense T for such a matching: T[s][s] = 1 if partner[s] == s, else T[s][s] = T[s][p] = 0.5. */
+int hadpsgd_oracle_mixing_matrix_matching(int S, const int32_t* partner /*[S]*/, double* T /*[S*S]*/);
 
 /* The same algorithm carried in double (state in double, gradients widened
  * exactly).  Used by the closed-form pins and to derive the fp32 tolerance.  */

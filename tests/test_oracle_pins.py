@@ -236,6 +236,216 @@ def test_eq7_literal_variant_matches_dense(oracle_mod):
     assert np.allclose(w64, expect, rtol=1e-13, atol=1e-16)
 
 
+# ------------------------------------------------------------------ caller-supplied matchings, unmixed members,
+# ------------------------------------------------------------------ eq.-(7)-literal diagnostics (R8, R14)
+
+def matching_T(partner):
+    """Dense T_k for an arbitrary matching, built HERE from PAPER.md:66 generalised by DESIGN.md R8:
+    a pair (a,b) puts 0.5 at (a,a),(a,b),(b,a),(b,b); an unmixed member s has T_ss = 1."""
+    S = len(partner)
+    T = np.zeros((S, S))
+    for s, p in enumerate(partner):
+        if p == s:
+            T[s, s] = 1.0
+        else:
+            T[s, s] = T[s, p] = 0.5
+    return T
+
+
+def fl32_sub(a32, b32):
+    """Correctly rounded fp32 a - b: the difference of two fp32 values of nearby magnitude is exact
+    in double, so one rounding of the double result is the IEEE fp32 subtraction."""
+    return (a32.astype(np.float64) - b32.astype(np.float64)).astype(np.float32)
+
+
+def fl32_mul(a32, b32):
+    """Correctly rounded fp32 product: 24 x 24 significant bits fit a double exactly."""
+    return (np.asarray(a32, np.float32).astype(np.float64) * np.asarray(b32, np.float32).astype(np.float64)).astype(np.float32)
+
+
+MATCHINGS = [[1, 0, 2], [0, 1, 2, 3, 4], [4, 3, 2, 1, 0], [3, 1, 5, 0, 4, 2, 6], [1, 0, 3, 2, 5, 4, 7, 6],
+             [7, 2, 1, 4, 3, 6, 5, 0], [5, 4, 3, 2, 1, 0], [0]]
+
+
+@pytest.mark.parametrize("partner", MATCHINGS)
+@pytest.mark.parametrize("literal", [False, True])
+def test_matching_entry_against_dense_T(oracle_mod, partner, literal):
+    """hadpsgd_oracle_step_matching for any involution (odd S, unmixed members, non-neighbours):
+    weights bit for bit against the dense product with T built in this file, momentum against the
+    per-learner update, and all three diagnostics against numpy in double (R14):
+      default  W' = fl32(T (W - lr V'))             gap = |u_s - u_p|^2
+      literal  W' = fl32( fl32(T W) - fl32(lr V') ) gap = |w_s - w_p|^2 (OLD weights)
+    gap is exactly 0 for an unmixed member either way."""
+    S, G, P = len(partner), 3, 67
+    g, w, v = rand((S, G, P), 200 + S, 1e-3), rand((S, P), 201 + S, 0.05), rand((S, P), 202 + S, 0.01)
+    w_old = w.copy()
+    T = matching_T(partner)
+    assert np.array_equal(oracle_mod.mixing_matrix_matching(partner), T)
+    assert np.array_equal(T, T.T) and np.array_equal(T.sum(0), np.ones(S)) and np.array_equal(T @ T, T)
+    acc = g[:, 0].copy()
+    for k in range(1, G):
+        acc = acc + g[:, k]
+    gbar = acc * (np.float32(1.0) / np.float32(G))
+    vn = np.float32(MU) * v + gbar
+    t = fl32_mul(np.float32(LR), vn)
+    if literal:
+        m = (T @ w_old.astype(np.float64)).astype(np.float32)      # 0.5a+0.5b exact in double, one rounding
+        expect = fl32_sub(m, t)
+        a = w_old
+    else:
+        u = fl32_sub(w_old, t)
+        expect = (T @ u.astype(np.float64)).astype(np.float32)
+        a = u
+    flags = oracle_mod.EQ7_LITERAL if literal else 0
+    d = oracle_mod.step(g, w, v, LR, MU, 0, flags=flags, diag=True, partner=partner)
+    assert np.array_equal(bits(v), bits(vn))
+    assert np.array_equal(bits(w), bits(expect))
+    pt = np.asarray(partner)
+    a64 = a.astype(np.float64)
+    assert np.allclose(d["gsq"], (gbar.astype(np.float64) ** 2).sum(1), rtol=1e-12, atol=0)
+    assert np.allclose(d["wsq"], (expect.astype(np.float64) ** 2).sum(1), rtol=1e-12, atol=0)
+    assert np.allclose(d["gap"], ((a64 - a64[pt]) ** 2).sum(1), rtol=1e-12, atol=0)
+    for s in range(S):
+        if partner[s] == s:
+            assert d["gap"][s] == 0.0                              # exactly, not merely small
+        else:
+            assert d["gap"][s] > 0 and d["gap"][s] == d["gap"][partner[s]]
+
+
+@pytest.mark.parametrize("literal", [False, True])
+def test_matching_entry_f64_shadow(oracle_mod, literal):
+    partner = [3, 1, 5, 0, 4, 2, 6]
+    S, G, P = 7, 2, 41
+    g, w, v = rand((S, G, P), 210, 1e-3), rand((S, P), 211, 0.05), rand((S, P), 212, 0.01)
+    w64, v64 = w.astype(np.float64), v.astype(np.float64)
+    lr, mu = float(np.float32(LR)), float(np.float32(MU))
+    vn = mu * v64 + g.astype(np.float64).mean(1)
+    T = matching_T(partner)
+    expect = T @ w64 - lr * vn if literal else T @ (w64 - lr * vn)
+    flags = oracle_mod.EQ7_LITERAL if literal else 0
+    oracle_mod.step_f64(g, w64, v64, lr, mu, 0, flags=flags, partner=partner)
+    assert np.allclose(w64, expect, rtol=1e-13, atol=1e-17) and np.allclose(v64, vn, rtol=1e-14, atol=0)
+    oracle_mod.step(g, w, v, LR, MU, 0, flags=flags, partner=partner)
+    assert np.all(np.abs(w - expect) <= 1e-6 + 1e-5 * np.abs(expect))
+
+
+def test_matching_entry_equals_ring_entry_on_ring_matchings(oracle_mod):
+    S, G, P = 8, 2, 129
+    for k in (0, 1):
+        for flags in (0, oracle_mod.EQ7_LITERAL):
+            g, w, v = rand((S, G, P), 220 + k, 1e-3), rand((S, P), 221, 0.05), rand((S, P), 222, 0.01)
+            w2, v2 = w.copy(), v.copy()
+            d1 = oracle_mod.step(g, w, v, LR, MU, k, flags=flags, diag=True)
+            d2 = oracle_mod.step(g, w2, v2, LR, MU, 99, flags=flags, diag=True, partner=oracle_mod.partner(S, k))
+            assert np.array_equal(bits(w), bits(w2)) and np.array_equal(bits(v), bits(v2))
+            for name in ("gsq", "wsq", "gap"):
+                assert np.array_equal(d1[name], d2[name])
+
+
+def test_matching_entry_rejects_non_involutions(oracle_mod):
+    g, w, v = np.zeros((3, 1, 4), np.float32), np.zeros((3, 4), np.float32), np.zeros((3, 4), np.float32)
+    for bad in ([1, 2, 0], [1, 1, 2], [0, 1, 3], [-1, 1, 2]):
+        with pytest.raises(ValueError):
+            oracle_mod.step(g, w, v, LR, MU, 0, partner=bad)
+        with pytest.raises(ValueError):
+            oracle_mod.mixing_matrix_matching(bad)
+    with pytest.raises(ValueError):
+        oracle_mod.step(g, w, v, LR, MU, 0, partner=[0, 1])           # wrong length
+
+
+@pytest.mark.parametrize("literal", [False, True])
+def test_exact_rational_example_with_matching_and_diagnostics(oracle_mod, literal):
+    """Dyadic inputs for which EVERY fp32 and double operation is exact, S = 5 with one unmixed
+    member and a non-neighbour pair: weights, momentum AND the three diagnostics must equal the
+    exact rational values (fractions.Fraction) of
+        v' = mu v + (1/G) sum_g g
+        default: u = w - lr v' ; w'_s = (u_s + u_p)/2            ; gap = sum (u_s - u_p)^2
+        literal: w'_s = (w_s + w_p)/2 - lr v'_s  (PAPER.md:64)   ; gap = sum (w_s - w_p)^2
+        unmixed: w'_s = w_s - lr v'_s                            ; gap = 0
+        gsq = sum gbar^2 ; wsq = sum w'^2."""
+    F = Fraction
+    S, G, P = 5, 2, 3
+    partner = [3, 4, 2, 0, 1]                                # pairs (0,3), (1,4); 2 unmixed
+    lr, mu = F(1, 2), F(1, 4)
+    w = [[F(s * 8 + i * 3 - 7, 16) for i in range(P)] for s in range(S)]
+    v = [[F(-(s + 1) * (i + 2), 32) for i in range(P)] for s in range(S)]
+    g = [[[F((s * 5 + gg * 3 + i * 7) % 11 - 5, 8) for i in range(P)] for gg in range(G)] for s in range(S)]
+    wn = np.array([[float(x) for x in r] for r in w], np.float32)
+    vn = np.array([[float(x) for x in r] for r in v], np.float32)
+    gn = np.array([[[float(x) for x in r] for r in q] for q in g], np.float32)
+    d = oracle_mod.step(gn, wn, vn, float(lr), float(mu), 0, flags=oracle_mod.EQ7_LITERAL if literal else 0,
+                        diag=True, partner=partner)
+    gbar = [[sum(g[s][gg][i] for gg in range(G)) / G for i in range(P)] for s in range(S)]
+    v2 = [[mu * v[s][i] + gbar[s][i] for i in range(P)] for s in range(S)]
+    u = [[w[s][i] - lr * v2[s][i] for i in range(P)] for s in range(S)]
+    w2 = [[None] * P for _ in range(S)]
+    gap = [F(0)] * S
+    for s in range(S):
+        p = partner[s]
+        for i in range(P):
+            if literal:
+                w2[s][i] = (w[s][i] + w[p][i]) / 2 - lr * v2[s][i]
+            else:
+                w2[s][i] = (u[s][i] + u[p][i]) / 2
+        a = w if literal else u
+        gap[s] = sum((a[s][i] - a[p][i]) ** 2 for i in range(P))
+    for s in range(S):
+        for i in range(P):
+            assert F(float(vn[s, i])) == v2[s][i], (s, i)
+            assert F(float(wn[s, i])) == w2[s][i], (s, i)
+        assert F(float(d["gsq"][s])) == sum(x * x for x in gbar[s]), s
+        assert F(float(d["wsq"][s])) == sum(x * x for x in w2[s]), s
+        assert F(float(d["gap"][s])) == gap[s], s
+    assert gap[2] == 0 and gap[0] == gap[3] != 0 and gap[1] == gap[4] != 0
+    if literal:                                                  # pair members end up DIFFERENT (R3)
+        assert w2[0] != w2[3]
+    else:
+        assert w2[0] == w2[3] and w2[1] == w2[4]
+
+
+def test_eq7_literal_with_equal_pair_weights_is_plain_momentum_sgd(oracle_mod):
+    """T_k is doubly stochastic, so mixing columns that are already EQUAL changes nothing
+    (PAPER.md:66, :72).  With w_s == w_p in every pair, eq. (7) as printed therefore collapses to
+    each learner's own eq.-(3)+momentum update: the EQ7_LITERAL step must equal the unmixed step
+    bit for bit (this fixes the fp32 order: the mixed OLD weights are formed first, exactly, and
+    lr v' is subtracted once -- any other association rounds differently), and gap must be 0."""
+    S, G, P = 6, 2, 5001
+    partner = [1, 0, 3, 2, 5, 4]
+    base = rand((S // 2, P), 230, 0.05)
+    w = np.ascontiguousarray(np.repeat(base, 2, axis=0))
+    v, g = rand((S, P), 231, 0.01), rand((S, G, P), 232, 1e-3)
+    wa, va, wb, vb = w.copy(), v.copy(), w.copy(), v.copy()
+    da = oracle_mod.step(g, wa, va, LR, MU, 0, flags=oracle_mod.EQ7_LITERAL, diag=True, partner=partner)
+    db = oracle_mod.step(g, wb, vb, LR, MU, 0, flags=oracle_mod.NO_MIX, diag=True)
+    assert np.array_equal(bits(wa), bits(wb)) and np.array_equal(bits(va), bits(vb))
+    assert not da["gap"].any() and not db["gap"].any()
+    assert np.array_equal(da["wsq"], db["wsq"]) and np.array_equal(da["gsq"], db["gsq"])
+    assert np.all(da["wsq"] > 0) and np.all(da["gsq"] > 0)
+
+
+@pytest.mark.parametrize("case", ["no_mix", "S1", "identity_matching"])
+def test_unmixed_diagnostics(oracle_mod, case):
+    """T_k = I (NO_MIX, S = 1, or a matching of fixed points): gap is exactly 0, gsq and wsq are the
+    plain sums of squares in double, and w' = u."""
+    S = 1 if case == "S1" else 5
+    G, P = 4, 333
+    g, w, v = rand((S, G, P), 240, 1e-3), rand((S, P), 241, 0.05), rand((S, P), 242, 0.01)
+    acc = g[:, 0].copy()
+    for k in range(1, G):
+        acc = acc + g[:, k]
+    gbar = acc * np.float32(0.25)
+    vn = np.float32(MU) * v + gbar
+    u = fl32_sub(w, fl32_mul(np.float32(LR), vn))
+    if case == "identity_matching":
+        d = oracle_mod.step(g, w, v, LR, MU, 0, diag=True, partner=list(range(S)))
+    else:
+        d = oracle_mod.step(g, w, v, LR, MU, 1, flags=oracle_mod.NO_MIX if case == "no_mix" else 0, diag=True)
+    assert np.array_equal(bits(w), bits(u)) and np.array_equal(bits(v), bits(vn))
+    assert np.array_equal(d["gap"], np.zeros(S))
+    assert np.allclose(d["gsq"], (gbar.astype(np.float64) ** 2).sum(1), rtol=1e-12, atol=0)
+    assert np.allclose(d["wsq"], (u.astype(np.float64) ** 2).sum(1), rtol=1e-12, atol=0)
+
+
 # ------------------------------------------------------------------ consensus (PAPER.md:72)
 
 @pytest.mark.parametrize("S", [2, 4, 8, 16])
