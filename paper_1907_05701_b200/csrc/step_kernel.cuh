@@ -435,8 +435,11 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     }
 
     if constexpr (DIAG) {
-        // last block to arrive reduces all block partials in a fixed order
+        // last block to arrive reduces all block partials in a fixed order.  Order matters: every
+        // thread's partial stores, then its fence, then a block barrier, and only then the ticket --
+        // otherwise warp 0 could publish the ticket before another warp's partials are out.
         __threadfence();
+        __syncthreads();
         if (tid == 0) {
             unsigned int t = atomicAdd(a.ticket, 1u);
             s_last = (t == gridDim.x - 1) ? 1u : 0u;

@@ -58,13 +58,12 @@ def run_both(H, oracle_mod, S, G, seg_len, steps, *, bf16=False, flags=0, seed=1
         og = problem.host_grads(seed, k, S, G, 0, P, dist, bf16=bf16)
         if matching is not None:
             h.hadpsgd_step_matching(lr, mu, k, matching(k))
+            od = oracle_mod.step(og, ow, ov, lr, mu, k, flags=oflags & ~oracle_mod.NO_MIX, diag=True, partner=matching(k))
         else:
             h.hadpsgd_step(lr, mu, k)
-        od = oracle_mod.step(og, ow, ov, lr, mu, k, flags=oflags, diag=True)
-        if check_diag and not (flags & H.NO_DIAG) and matching is None:
-            gd = h.hadpsgd_diagnostics()
-            for name in ("gsq", "wsq", "gap"):
-                assert np.allclose(gd[name], od[name], rtol=1e-4, atol=1e-30), (name, k, gd[name], od[name])
+            od = oracle_mod.step(og, ow, ov, lr, mu, k, flags=oflags, diag=True)
+        if check_diag and not (flags & H.NO_DIAG):
+            assert_diag(h.hadpsgd_diagnostics(), od, k)
     torch.cuda.synchronize()
     gw = np.stack([h.hadpsgd_weights(s)[nat].cpu().numpy() for s in range(S)])
     gv = np.stack([h.hadpsgd_momentum(s)[nat].cpu().numpy() for s in range(S)])
@@ -75,6 +74,14 @@ def run_both(H, oracle_mod, S, G, seg_len, steps, *, bf16=False, flags=0, seed=1
             assert not h.hadpsgd_weights(s)[mask].any() and not h.hadpsgd_momentum(s)[mask].any()
     h.close()
     return gw, gv, ow, ov
+
+
+def assert_diag(gd, od, k=0):
+    """a5 against the oracle's double accumulators (R14, R16): relative 1e-4; a gap the
+    oracle reports as exactly 0 (unmixed member) must be exactly 0 on the GPU too."""
+    for name in ("gsq", "wsq", "gap"):
+        assert np.allclose(gd[name], od[name], rtol=1e-4, atol=1e-30), (name, k, gd[name], od[name])
+    assert np.array_equal(gd["gap"] == 0.0, od["gap"] == 0.0), (k, gd["gap"], od["gap"])
 
 
 def assert_parity(gw, gv, ow, ov, exact):
@@ -185,8 +192,10 @@ def test_uniform_sweep_points(H, oracle_mod):
     """BASELINE.json configs[4] (bandwidth sweep) sample points small enough for a full
     oracle run: flat fp32, uniform grads in [-1e-3, 1e-3]."""
     for P, S, G in ((1 << 10, 2, 2), (1 << 12, 16, 8), (1 << 14, 4, 4), (1 << 16, 8, 2), (1 << 18, 2, 8)):
-        gw, gv, ow, ov = run_both(H, oracle_mod, S, G, [P], 3, flags=H.DETERMINISTIC, seed=P + S + G, dist="uniform")
-        assert_parity(gw, gv, ow, ov, True)
+        for exact in (True, False):                        # deterministic: bits; default (FMA): tolerance
+            gw, gv, ow, ov = run_both(H, oracle_mod, S, G, [P], 3, flags=H.DETERMINISTIC if exact else 0,
+                                      seed=P + S + G, dist="uniform")
+            assert_parity(gw, gv, ow, ov, exact)
 
 
 # ------------------------------------------------------------------------------- shared pair storage
@@ -255,13 +264,8 @@ def test_share_pair_weights_with_custom_matchings_and_unpaired_members(H, oracle
     for k, partner in enumerate(matchings):
         problem.fill_grads(h, seed, k)
         h.hadpsgd_step_matching(LR, MU, k, partner)
-        og = problem.host_grads(seed, k, S, G, 0, P)
-        groups = {tuple(sorted({s, partner[s]})) for s in range(S)}
-        for grp in groups:                                         # the step is pair-local: oracle per sub-ring
-            grp = list(grp)
-            w, v, g = ow[grp].copy(), ov[grp].copy(), np.ascontiguousarray(og[grp])
-            oracle_mod.step(g, w, v, LR, MU, 0)
-            ow[grp], ov[grp] = w, v
+        od = oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k, diag=True, partner=partner)
+        assert_diag(h.hadpsgd_diagnostics(), od, k)
         gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
         gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
         assert np.array_equal(bits(gw), bits(ow)) and np.array_equal(bits(gv), bits(ov)), k
@@ -302,9 +306,9 @@ def test_share_pair_weights_graph_replay_from_steady_state(H, oracle_mod, torch_
 # ------------------------------------------------------------------------------- API behaviour
 
 def test_custom_matching_and_unpaired(H, oracle_mod):
-    """hadpsgd_step_matching (row f1): caller-supplied matching, including unpaired members.
-    Oracle side: the step is element-wise and pair-local, so it is assembled from oracle runs
-    on the sub-rings {pair} (S=2) and {single} (S=1)."""
+    """hadpsgd_step_matching (row f1): caller-supplied matching, including unpaired members, against
+    the oracle's own matching entry (weights, momentum and all three diagnostics; two launches --
+    pairs then singles -- feed one diagnostics record)."""
     import torch
     from fixtures import problem
     S, G, P, seed = 7, 2, 20_000, 81                  # odd S: only possible with unpaired members
@@ -314,11 +318,8 @@ def test_custom_matching_and_unpaired(H, oracle_mod):
     problem.fill_grads(h, seed, 0)
     h.hadpsgd_step_matching(LR, MU, 0, partner)
     ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
-    og = problem.host_grads(seed, 0, S, G, 0, P)
-    for grp in ([0, 3], [2, 5], [1], [4], [6]):
-        w, v, g = ow[grp].copy(), ov[grp].copy(), np.ascontiguousarray(og[grp])
-        oracle_mod.step(g, w, v, LR, MU, 0)
-        ow[grp], ov[grp] = w, v
+    od = oracle_mod.step(problem.host_grads(seed, 0, S, G, 0, P), ow, ov, LR, MU, 0, diag=True, partner=partner)
+    assert_diag(h.hadpsgd_diagnostics(), od)
     torch.cuda.synchronize()
     gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
     gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
@@ -326,6 +327,54 @@ def test_custom_matching_and_unpaired(H, oracle_mod):
     with pytest.raises(H.HadpsgdError):
         h.hadpsgd_step_matching(LR, MU, 0, [1, 2, 0, 3, 4, 5, 6])  # not an involution
     h.close()
+
+
+MATCHING_SEQ = [[3, 1, 5, 0, 4, 2, 6], [1, 0, 3, 2, 5, 4, 6], [0, 1, 2, 3, 4, 5, 6], [6, 2, 1, 4, 3, 5, 0]]
+
+
+@pytest.mark.parametrize("flagname", [None, "EQ7_LITERAL"])
+@pytest.mark.parametrize("bf16", [False, True])
+@pytest.mark.parametrize("exact", [True, False])
+def test_matching_sequences_with_diagnostics(H, oracle_mod, flagname, bf16, exact):
+    """Caller-supplied matchings over several steps (odd S, non-neighbour pairs, unmixed members, the
+    identity), default and eq.-(7)-literal: w, v and every step's diagnostics against the oracle's
+    matching entry."""
+    flags = (H.DETERMINISTIC if exact else 0) | (getattr(H, flagname) if flagname else 0)
+    gw, gv, ow, ov = run_both(H, oracle_mod, 7, 3, ODD_TABLE, len(MATCHING_SEQ), bf16=bf16, flags=flags, seed=171,
+                              v0_sd=0.01, matching=lambda k: MATCHING_SEQ[k])
+    assert_parity(gw, gv, ow, ov, exact)
+
+
+def test_max_S_unmixed_diagnostics_span_several_launches(H, oracle_mod):
+    """S = 512 unmixed super-learners = 512 single items > kMaxWork: several launches feed one
+    diagnostics record (gap exactly 0 everywhere)."""
+    gw, gv, ow, ov = run_both(H, oracle_mod, 512, 2, [3_001], 2, flags=H.DETERMINISTIC | H.NO_MIX, seed=52)
+    assert_parity(gw, gv, ow, ov, True)
+
+
+def test_diagnostics_stress_large_grids(H, oracle_mod):
+    """Many work items (S = 32: 16 pairs, so several warps write block partials), the largest
+    persistent grid (16 blocks/SM), many steps: diagnostics must equal the oracle's every step and be
+    bitwise identical between two runs (the ticketed last-block reduction has a fixed order)."""
+    from fixtures import problem
+    S, G, P, seed, steps = 32, 2, 40_003, 181, 12
+    runs = []
+    for rep in range(2):
+        h = H.Hadpsgd(S, G, [P], H.F32, 0)
+        h.hadpsgd_set_launch(16)
+        problem.fill_weights(h, seed)
+        ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+        rec = []
+        for k in range(steps):
+            problem.fill_grads(h, seed, k)
+            h.hadpsgd_step(LR, MU, k)
+            gd = h.hadpsgd_diagnostics()
+            if rep == 0:
+                assert_diag(gd, oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k, diag=True), k)
+            rec.append(np.concatenate([gd["gsq"], gd["wsq"], gd["gap"]]))
+        runs.append(np.stack(rec))
+        h.close()
+    assert np.array_equal(runs[0], runs[1])
 
 
 @pytest.mark.parametrize("share", [False, True])
@@ -358,12 +407,16 @@ def test_host_gradient_path_equals_resident_path(H, oracle_mod, share):
     assert np.array_equal(bits(outs[0][0]), bits(outs[1][0])) and np.array_equal(bits(outs[0][1]), bits(outs[1][1]))
     for name in ("gsq", "wsq", "gap"):
         assert np.allclose(outs[0][2][name], outs[1][2][name], rtol=1e-12)
-    # sampled window against the oracle
-    lo, hi = P - 5000, P
-    ow, ov = problem.host_weights(seed, S, lo, hi), np.zeros((S, hi - lo), np.float32)
-    for k in range(2):
-        oracle_mod.step(problem.host_grads(seed, k, S, G, lo, hi), ow, ov, LR, MU, k)
-    assert np.array_equal(bits(outs[1][0][:, lo:hi]), bits(ow))
+    # against the oracle: windows around every chunk boundary of the host path (8 Mi elements), the
+    # start, the ragged end and two interior stretches -- 1.3 M elements per buffer in all
+    chunk = 8 << 20
+    wins = [(0, 200_000), (chunk - 100_000, chunk + 100_000), (2 * chunk - 100_000, 2 * chunk + 100_000),
+            (P - 200_000, P), (3_000_000, 3_250_000), (12_000_000, 12_250_000)]
+    for lo, hi in wins:
+        ow, ov = problem.host_weights(seed, S, lo, hi), np.zeros((S, hi - lo), np.float32)
+        for k in range(2):
+            oracle_mod.step(problem.host_grads(seed, k, S, G, lo, hi), ow, ov, LR, MU, k)
+        assert np.array_equal(bits(outs[1][0][:, lo:hi]), bits(ow)) and np.array_equal(bits(outs[1][1][:, lo:hi]), bits(ov))
 
 
 @pytest.mark.parametrize("exact", [True, False])
@@ -653,11 +706,76 @@ def full_size_parity(H, oracle_mod, name, *, exact, n_win=6, width=8192, extra_f
 def test_config1_swb300_full_size(H, oracle_mod):
     """configs[1]: 94,797,312 params flat fp32, S=16, G=4, 20 steps (36.4 GB resident)."""
     full_size_parity(H, oracle_mod, "swb300", exact=True)
+    full_size_parity(H, oracle_mod, "swb300", exact=False, n_win=3)      # default (FMA) mode: tolerance
 
 
 def test_config2_swb2000_full_size_exact(H, oracle_mod):
     """configs[2] (headline): 145,145,344 params flat fp32, S=16, G=4, 20 steps (55.7 GB)."""
     full_size_parity(H, oracle_mod, "swb2000", exact=True)
+
+
+def test_config2_swb2000_whole_buffer_every_element(H, oracle_mod, torch_cuda):
+    """configs[2] (headline), launch configuration of bench.py, deterministic mode: EVERY element of
+    every weight and momentum buffer after 2 steps (both ring parities) against the oracle, bit for
+    bit.  The oracle stays single-threaded; it is run on disjoint 1 Mi-element windows by one host
+    thread per core (the C call releases the GIL).  Oracle inputs come from the device twin of the
+    seeded generator (bit-compared with the numpy one in test_device_generator_matches_host),
+    generated per window and copied down -- 100 GB of numpy hashing would take minutes."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    torch = torch_cuda
+    from fixtures import device, generator as gen, problem, shapes
+    cfg = shapes.CONFIGS["swb2000"]
+    S, G, P, steps, seed = cfg["S"], cfg["G"], int(sum(cfg["seg_len"])), 2, 4242
+    h = H.Hadpsgd(S, G, cfg["seg_len"], H.F32, H.DETERMINISTIC)
+    assert h.P_padded == P
+    problem.fill_weights(h, seed)
+    for k in range(steps):
+        problem.fill_grads(h, seed, k)
+        h.hadpsgd_step(LR, MU, k)
+    torch.cuda.synchronize()
+    assert h.hadpsgd_launch_count() == steps
+    n_threads = os.cpu_count() or 1
+    W = 1 << 20
+    compared = {"w": 0, "v": 0}
+
+    def check(lo, hi, w0, grads, gw, gv):
+        ow, ov = w0, np.zeros((S, hi - lo), np.float32)
+        for k in range(steps):
+            oracle_mod.step(grads[k], ow, ov, LR, MU, k)
+        bad_w, bad_v = int(np.sum(bits(gw) != bits(ow))), int(np.sum(bits(gv) != bits(ov)))
+        return lo, hi, bad_w, bad_v
+
+    dev_w0 = torch.empty((S, W), dtype=torch.float32, device="cuda")
+    dev_g = torch.empty((steps, S, G, W), dtype=torch.float32, device="cuda")
+    futures = []
+    with ThreadPoolExecutor(max_workers=n_threads) as pool:
+        for lo in range(0, P, W):
+            hi = min(lo + W, P)
+            n = hi - lo
+            for s in range(S):
+                device.fill(dev_w0[s], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, s, 0), "normal", 0.05, elem_offset=lo, n=n)
+                for k in range(steps):
+                    for g in range(G):
+                        device.fill(dev_g[k, s, g], gen.stream_key(seed, gen.STREAM_GRAD, k, s, g), "normal", 1e-3,
+                                    elem_offset=lo, n=n)
+            w0 = np.ascontiguousarray(dev_w0[:, :n].cpu().numpy())
+            grads = [np.ascontiguousarray(dev_g[k, :, :, :n].cpu().numpy()) for k in range(steps)]
+            gw = np.stack([h.hadpsgd_weights(s)[lo:hi].cpu().numpy() for s in range(S)])
+            gv = np.stack([h.hadpsgd_momentum(s)[lo:hi].cpu().numpy() for s in range(S)])
+            futures.append(pool.submit(check, lo, hi, w0, grads, gw, gv))
+            while len(futures) > 2 * n_threads:           # bound the host memory in flight
+                lo_, hi_, bw, bv = futures.pop(0).result()
+                assert bw == 0 and bv == 0, (lo_, hi_, bw, bv)
+                compared["w"] += S * (hi_ - lo_); compared["v"] += S * (hi_ - lo_)
+        for f in futures:
+            lo_, hi_, bw, bv = f.result()
+            assert bw == 0 and bv == 0, (lo_, hi_, bw, bv)
+            compared["w"] += S * (hi_ - lo_); compared["v"] += S * (hi_ - lo_)
+    assert compared["w"] == S * P and compared["v"] == S * P       # every element of every buffer
+    h.close()
+    del dev_w0, dev_g
+    torch.cuda.empty_cache()
 
 
 def test_config2_swb2000_full_size_default_mode(H, oracle_mod):
