@@ -9,9 +9,17 @@ the achieved HBM GB/s in `roofline`.  Default workload = BASELINE.json configs[2
 145,145,344-parameter SWB-2000-shaped flat fp32 buffer with S=16 super-learners x G=4
 learners (55.7 GB resident), which is the configuration the metric is quoted on.
 
-N > 1 (torchrun): the path is element-wise independent, so every rank owns one P-element
-range of an N*P-parameter model (no data-path collective, "scaling": "weak"); only the few
-diagnostic doubles are all-reduced, after the timed region.
+N > 1 (torchrun), --partition:
+  range (default)   ONE model of the configured size: rank r owns the parameter range
+                    hadpsgd_shard_range(P, N, r) of every buffer (the method is element-wise, so there
+                    is no data-path collective; only the few diagnostic doubles are all-reduced, after
+                    the timed region).  Total work is fixed: "scaling": "strong".
+  superlearner      the paper's topology: rank r owns S/N super-learners with all
+                    P parameters; a pair whose members live on two GPUs is mixed by peer reads of the
+                    partner's stage buffer inside the fused kernel (HADPSGD_PEER, CUDA IPC mappings),
+                    4*P bytes per pending member per step over NVLink; the epoch barrier between steps
+                    is a one-element NCCL all-reduce on the kernel's stream.  "scaling": "strong".
+  weak              every rank runs its own problem of the configured size ("scaling": "weak").
 
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
 workload on the host cores; rank 0 only.
@@ -32,13 +40,38 @@ METRIC = "learner_params_updated_per_sec"
 UNIT = "learner-params/s"
 LR, MU = 0.1, 0.9
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the
-# `ncu --set full` capture summarised in profiles/ (bytes; None until a capture exists)
-NCU_TRAFFIC_BYTES = {"swb2000": 74.284e9, "swb300": 48.502e9, "swb2000_ragged_bf16": 37.123e9, "paper_literal": 16.536e9}
-NCU_TRAFFIC_SHARED = {"swb2000": 66.555e9, "swb2000_ragged_bf16": 33.285e9}     # same, with HADPSGD_SHARE_PAIR_WEIGHTS (profiles/r01_share_pair_weights.md)
-NCU_TRAFFIC_SOURCE = {"swb2000": "profiles/r01_step_kernel_ncu.md (dram__bytes_read.sum 55.737 GB + dram__bytes_write.sum 18.545 GB)",
-                      "swb300": "profiles/r01_traffic_other_workloads.md", "swb2000_ragged_bf16": "profiles/r01_traffic_other_workloads.md",
-                      "paper_literal": "profiles/r01_traffic_other_workloads.md"}
+PCIE_GEN5_X16_GBS = 64.0        # nominal per direction; the e2e leg reports its fraction of this
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+KERNEL_SOURCES = ["paper_1907_05701_b200/csrc/step_kernel.cuh", "paper_1907_05701_b200/csrc/step_dispatch.cuh"]
+
+
+def kernel_source_sha():
+    import hashlib
+    h = hashlib.sha256()
+    for rel in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, flags_text, emit):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed
+    `ncu --set full` captures (profiles/r02_traffic.csv; the .md beside it names the commands).  Only a
+    capture taken on THIS kernel source (sha of step_kernel.cuh + step_dispatch.cuh) for this workload
+    and these flags counts; anything else is None."""
+    import csv
+    want = (workload, ",".join(sorted(filter(None, (t.strip() for t in flags_text.split(","))))), "1" if emit else "0")
+    try:
+        with open(TRAFFIC_CSV) as f:
+            for row in csv.DictReader(f):
+                if (row["workload"], row["flags"], row["emit_bf16"]) == want:
+                    if row["kernel_source_sha16"] != kernel_source_sha():
+                        return None, f"profiles/r02_traffic.csv holds a capture of another kernel source ({row['kernel_source_sha16']})"
+                    return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), \
+                        f"profiles/r02_traffic.csv: {row['kernel']} at commit {row['commit']} (read {row['dram_bytes_read']} B + write {row['dram_bytes_write']} B)"
+    except Exception as e:                      # no capture file: say so, never guess
+        return None, f"no capture: {e}"
+    return None, "no capture for this workload / flags"
 
 
 def parse_args():
@@ -52,15 +85,20 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-elems", type=int, default=1 << 22)
-    ap.add_argument("--cpu-sample-steps", type=int, default=20)
+    ap.add_argument("--cpu-sample-steps", type=int, default=10)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--flags", default="", help="comma list: deterministic,no_diag,no_mix,eq7,share")
     ap.add_argument("--no-share-leg", action="store_true", help="skip the extra HADPSGD_SHARE_PAIR_WEIGHTS leg")
     ap.add_argument("--emit-bf16", action="store_true",
                     help="also write the bf16 working copy of the weights every step (row f2; +2 B/param)")
+    ap.add_argument("--partition", default="range", choices=["range", "superlearner", "weak"],
+                    help="how N > 1 GPUs share the work (ignored for N = 1)")
+    ap.add_argument("--no-ceiling", action="store_true", help="skip the pure-read / pure-write membench legs")
+    ap.add_argument("--cpu-repeats", type=int, default=3)
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[4]: bandwidth sweep over P, S, G (one JSON line per point)")
     ap.add_argument("--sweep-md", default="", help="also write the sweep as a markdown table to this path")
+    ap.add_argument("--sweep-max-log2", type=int, default=28, help="only sweep points with P <= 2^N")
     return ap.parse_args()
 
 
@@ -196,36 +234,80 @@ def host_cpu():
     return model, os.cpu_count()
 
 
-def time_oracle(cfg, n_elems, steps, warmup=1):
+def time_oracle(cfg, n_elems, steps, warmup=1, repeats=1, lo=0):
     """The oracle as it stands (single thread, oracle/hadpsgd_oracle.cpp) on a bounded sample:
-    the first n_elems parameters of every buffer of the workload (the method is element-wise
-    independent, so a window is the same work per parameter).  Returns seconds per step."""
+    n_elems parameters (from `lo`) of every buffer of the workload (the method is element-wise
+    independent, so a window is the same work per parameter).  Returns (seconds per step of each
+    repeat, n)."""
     import numpy as np
     import oracle
     from fixtures import problem
     S, G = cfg["S"], cfg["G"]
-    n = min(n_elems, cfg["P"])
+    n = min(n_elems, cfg["P"] - lo)
     bf16 = cfg["grad"] == "bf16"
-    w = problem.host_weights(7, S, 0, n)
+    w = problem.host_weights(7, S, lo, lo + n)
     v = np.zeros((S, n), np.float32)
-    g = problem.host_grads(7, 0, S, G, 0, n, cfg["dist"], bf16=bf16)
+    g = problem.host_grads(7, 0, S, G, lo, lo + n, cfg["dist"], bf16=bf16)
     for k in range(warmup):
         oracle.step(g, w, v, LR, MU, k, diag=True)
-    t0 = time.perf_counter()
-    for k in range(steps):
-        oracle.step(g, w, v, LR, MU, warmup + k, diag=True)
-    dt = (time.perf_counter() - t0) / max(steps, 1)
-    return dt, n
+    times = []
+    for r in range(max(repeats, 1)):
+        t0 = time.perf_counter()
+        for k in range(steps):
+            oracle.step(g, w, v, LR, MU, warmup + k, diag=True)
+        times.append((time.perf_counter() - t0) / max(steps, 1))
+    return times, n
 
 
-def cpu_baseline(cfg, n_elems, steps):
-    dt, n = time_oracle(cfg, n_elems, steps)
+def time_oracle_all_cores(cfg, n_elems_per_thread, steps):
+    """The same single-threaded oracle, one instance per hardware thread, each on its own disjoint
+    element window (the C call releases the GIL).  Returns (seconds for `steps` steps, threads, n)."""
+    import numpy as np
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+    from fixtures import problem
+    S, G = cfg["S"], cfg["G"]
+    threads = os.cpu_count() or 1
+    n = min(n_elems_per_thread, cfg["P"] // threads)
+    bf16 = cfg["grad"] == "bf16"
+    work = []
+    for t in range(threads):
+        lo = t * n
+        work.append((problem.host_grads(7, 0, S, G, lo, lo + n, cfg["dist"], bf16=bf16),
+                     problem.host_weights(7, S, lo, lo + n), np.zeros((S, n), np.float32)))
+
+    def run(item):
+        g, w, v = item
+        for k in range(steps):
+            oracle.step(g, w, v, LR, MU, k, diag=True)
+
+    with ThreadPoolExecutor(max_workers=threads) as pool:
+        list(pool.map(run, [(g, w.copy(), v.copy()) for g, w, v in work]))     # warm-up pass
+        t0 = time.perf_counter()
+        list(pool.map(run, work))
+        dt = time.perf_counter() - t0
+    return dt, threads, n
+
+
+def cpu_baseline(cfg, n_elems, steps, repeats=3, all_cores=True):
+    """`value` = the best of `repeats` repeats of the single-threaded oracle (its contract); the spread
+    of the repeats is reported next to it, and -- optionally -- the same oracle run by every hardware
+    thread on disjoint windows."""
+    times, n = time_oracle(cfg, n_elems, steps, repeats=repeats)
     model, ncpu = host_cpu()
-    return {"value": cfg["S"] * cfg["G"] * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"first {n} of {cfg['P']} params of every buffer (S={cfg['S']}, G={cfg['G']}), "
-                      f"{steps} steps after 1 warm-up, diagnostics on; single thread; host has {ncpu} logical CPUs ({model})",
-            "gb_per_s": cfg["S"] * n * (cfg["G"] * cfg["b_g"] + 16) / dt / 1e9,
-            "ms_per_step_sample": dt * 1e3}
+    per = cfg["S"] * cfg["G"] * n
+    best = min(times)
+    out = {"value": per / best, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"first {n} of {cfg['P']} params of every buffer (S={cfg['S']}, G={cfg['G']}), best of {len(times)} "
+                     f"repeats of {steps} steps after 1 warm-up, diagnostics on; single thread; host has {ncpu} logical CPUs ({model})",
+           "repeats": [per / t for t in times], "spread": (max(times) - min(times)) / min(times),
+           "gb_per_s": cfg["S"] * n * (cfg["G"] * cfg["b_g"] + 16) / best / 1e9,
+           "ms_per_step_sample": best * 1e3}
+    if all_cores:
+        dt, threads, m = time_oracle_all_cores(cfg, 1 << 18, 5)
+        out["all_cores"] = {"value": cfg["S"] * cfg["G"] * m * threads * 5 / dt, "unit": UNIT, "cores": threads,
+                            "sample": f"{threads} threads, each the single-threaded oracle on its own {m}-param window, 5 steps"}
+    return out
 
 
 def run_reference(args):
@@ -233,7 +315,8 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     cfg = workload(args.workload)
-    dt, n = time_oracle(cfg, args.cpu_sample_elems, args.steps, warmup=min(args.warmup, 2))
+    times, n = time_oracle(cfg, args.cpu_sample_elems, args.steps, warmup=min(args.warmup, 2))
+    dt = times[0]
     model, ncpu = host_cpu()
     value = cfg["S"] * cfg["G"] * n / dt
     sample = (f"each step = first {n} of {cfg['P']} params of every buffer (S={cfg['S']}, G={cfg['G']}); "
@@ -333,12 +416,119 @@ def time_e2e_steps(torch, dist, h, cfg, steps, warmup=1):
     return max(dev, wall), S * G * nbytes, 3 * S * 8, note
 
 
+def make_problem(H, torch, dist, args, cfg, flags, local, rank, world):
+    """Builds this rank's handle for the chosen partition and fills it.  Returns (handle, info)."""
+    from fixtures import device, generator as gen, problem
+    S, G, P = cfg["S"], cfg["G"], cfg["P"]
+    gdt = H.BF16 if cfg["grad"] == "bf16" else H.F32
+    wdt = H.BF16 if args.emit_bf16 else H.F32
+    part = args.partition if world > 1 else "single"
+    dist_name = cfg["dist"]
+    if part in ("single", "weak"):
+        h = H.Hadpsgd(S, G, cfg["seg_len"], gdt, flags, device=local, working_dtype=wdt)
+        seed = 2000 + rank            # weak: every rank is its own problem
+        problem.fill_weights(h, seed)
+        problem.fill_grads(h, seed, 0, dist_name)
+        info = {"units": S * G * P, "scaling": "weak",
+                "parallelism": "single GPU" if world == 1 else f"weak: {world} independent problems of the configured size, no collective"}
+        return h, info
+    if part == "range":
+        # ONE model: rank r owns the element range [lo, hi) of every buffer (hadpsgd_shard_range)
+        lay = H.hadpsgd_layout(S, G, cfg["seg_len"], gdt, wdt)
+        assert lay["P_padded"] == P, "--partition range needs a segment table without padding (all BLSTM tables are)"
+        lo, hi = H.hadpsgd_shard_range(P, world, rank)
+        h = H.Hadpsgd(S, G, [hi - lo], gdt, flags, device=local, working_dtype=wdt)
+        seed = 2000
+        for s_ in range(S):
+            device.fill(h.hadpsgd_weights(s_)[:hi - lo], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, s_, 0), "normal", 0.05,
+                        elem_offset=lo)
+            for g_ in range(G):
+                device.fill(h.hadpsgd_grads(s_, g_)[:hi - lo], gen.stream_key(seed, gen.STREAM_GRAD, 0, s_, g_), dist_name, 1e-3,
+                            elem_offset=lo)
+        info = {"units": S * G * (hi - lo), "scaling": "strong", "shard": [lo, hi],
+                "parallelism": f"range: one {P}-parameter model, rank r owns hadpsgd_shard_range(P, {world}, r) of every buffer; "
+                               "no data-path collective (diagnostics all-reduced after the timed region)"}
+        return h, info
+    # superlearner: rank r owns S/world super-learners with all P parameters (PAPER.md:84, :88)
+    assert S % world == 0, "--partition superlearner needs S divisible by the number of GPUs"
+    assert not args.emit_bf16 and not (flags & (H.SHARE_PAIR_WEIGHTS | H.EQ7_LITERAL)), "peer mode: no emit / share / eq7"
+    S_l = S // world
+    rank_begin = [r * S_l for r in range(world + 1)]
+    h = H.Hadpsgd(S_l, G, cfg["seg_len"], gdt, flags | H.PEER, device=local, own_arena=True)
+    h.hadpsgd_peer_init(rank, world, rank_begin)
+    ipc, off = h.hadpsgd_peer_ipc_export()
+    mine = torch.tensor(list(ipc) + list(off.to_bytes(8, "little")), dtype=torch.uint8, device="cuda")
+    got = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(got, mine)
+    for r in range(world):
+        if r != rank:
+            raw = bytes(got[r].cpu().tolist())
+            h.hadpsgd_peer_ipc_attach(r, raw[:64], int.from_bytes(raw[64:], "little"))
+    seed = 2000
+    nat = problem.natural_offsets(h.seg_len)
+    for s_ in range(S_l):
+        sg = rank_begin[rank] + s_
+        for k_, n_ in enumerate(h.seg_len):
+            o_, _ = h.hadpsgd_segment(k_)
+            device.fill(h.hadpsgd_weights(s_)[o_:o_ + n_], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, sg, 0), "normal", 0.05,
+                        elem_offset=int(nat[k_]))
+            for g_ in range(G):
+                device.fill(h.hadpsgd_grads(s_, g_)[o_:o_ + n_], gen.stream_key(seed, gen.STREAM_GRAD, 0, sg, g_), dist_name, 1e-3,
+                            elem_offset=int(nat[k_]))
+    # expected NVLink traffic: every member whose ring partner lives on another GPU publishes u on the
+    # odd (or even) step and reads its partner's 4*P bytes at the next launch
+    strad = [sum(1 for sg in range(rank_begin[rank], rank_begin[rank + 1])
+                 if not rank_begin[rank] <= H.hadpsgd_pairing(S, k)[sg] < rank_begin[rank + 1]) for k in (0, 1)]
+    info = {"units": S_l * G * P, "scaling": "strong", "barrier": True,
+            "nvlink_read_bytes_per_rank_per_step": [strad[1] * 4 * P, strad[0] * 4 * P],   # [even step reads what the odd step left, odd step ...]
+            "parallelism": f"superlearner: rank r owns super-learners [{S_l}r, {S_l}(r+1)) of {S}; straddling pairs mixed by peer reads "
+                           f"of the partner's stage buffer inside the fused kernel (CUDA IPC); epoch barrier = 1-element NCCL all-reduce per step"}
+    return h, info
+
+
+def time_device_steps_barrier(torch, dist, h, steps, warmup, k0=0, sampler=None):
+    """As time_device_steps, for --partition superlearner: every step is followed by the epoch barrier (a
+    one-element all-reduce enqueued behind the kernel), inside the timed region."""
+    tok = torch.zeros(1, device="cuda")
+    for k in range(warmup):
+        h.hadpsgd_step(LR, MU, k0 + k)
+        dist.all_reduce(tok)
+    torch.cuda.synchronize()
+    dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if sampler is not None:
+        sampler.start()
+    ev0.record(h.stream)
+    for k in range(steps):
+        h.hadpsgd_step(LR, MU, k0 + warmup + k)
+        dist.all_reduce(tok)
+    ev1.record(h.stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler is not None else None
+    dist.barrier()
+    torch.cuda.synchronize()
+    return ev0.elapsed_time(ev1) / 1e3, clocks
+
+
+def mix_ceiling(torch, read_bytes, write_bytes):
+    """This box's pure-read and pure-write streaming rates (fixtures/membench.cu, the step kernel's access
+    shape) and the ceiling they imply for this kernel's byte mix: reads and writes share one DRAM bus, so
+    t >= read_bytes / BW_read + write_bytes / BW_write."""
+    from fixtures import device
+    r = device.membench(8 << 30, 12, write=False, reps=3)
+    w = device.membench(8 << 30, 4, write=True, reps=3)
+    t = read_bytes / (r * 1e9) + write_bytes / (w * 1e9)
+    return {"read_gbs": r, "write_gbs": w, "mix_gbs": (read_bytes + write_bytes) / t / 1e9,
+            "how": "fixtures/membench.cu: 12 read streams / 4 write streams, 32 B accesses, 148 x 256 threads, best of 3; "
+                   "mix = bytes / (read_bytes / read_gbs + write_bytes / write_gbs)"}
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
     import paper_1907_05701_b200 as H
-    from fixtures import problem
     H.lib()                                   # fail loudly if libhadpsgd.so is missing
 
     rank = int(os.environ.get("RANK", "0"))
@@ -355,19 +545,14 @@ def run_ours(args):
     cfg["emit"] = args.emit_bf16
     S, G, P = cfg["S"], cfg["G"], cfg["P"]
     flags = parse_flags(H, args.flags)
-    h = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags, device=local,
-                  working_dtype=H.BF16 if args.emit_bf16 else H.F32)
+    h, info = make_problem(H, torch, dist, args, cfg, flags, local, rank, world)
     if args.blocks_per_sm:
         h.hadpsgd_set_launch(args.blocks_per_sm)
-    # rank r owns parameters [r*P, (r+1)*P) of an N*P-parameter model: its own seed stream
-    seed = 2000 + rank
-    problem.fill_weights(h, seed)
-    problem.fill_grads(h, seed, 0, cfg["dist"])
     torch.cuda.synchronize()
+    timer = time_device_steps_barrier if info.get("barrier") else time_device_steps
 
     n0 = h.hadpsgd_launch_count()
-    secs, clocks = time_device_steps(torch, dist, h, args.steps, args.warmup,
-                                     sampler=ClockSampler(local) if rank == 0 else None)
+    secs, clocks = timer(torch, dist, h, args.steps, args.warmup, sampler=ClockSampler(local) if rank == 0 else None)
     launches = h.hadpsgd_launch_count() - n0 - args.warmup
     # a timed region that saw a hardware or thermal slowdown is rejected and measured again, once
     bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
@@ -378,28 +563,34 @@ def run_ours(args):
     if remeasured:
         time.sleep(5.0)
         n0 = h.hadpsgd_launch_count()
-        secs, clocks = time_device_steps(torch, dist, h, args.steps, args.warmup, k0=args.steps + args.warmup,
-                                         sampler=ClockSampler(local) if rank == 0 else None)
+        secs, clocks = timer(torch, dist, h, args.steps, args.warmup, k0=args.steps + args.warmup,
+                             sampler=ClockSampler(local) if rank == 0 else None)
         launches = h.hadpsgd_launch_count() - n0 - args.warmup
     if clocks is not None:
         clocks["remeasured_after_slowdown"] = remeasured
     diag = None if (flags & H.NO_DIAG) else h.hadpsgd_diagnostics()
 
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not info.get("barrier"):
         e_secs, h2d, d2h, note = time_e2e_steps(torch, dist, h, cfg, args.e2e_steps)
         e2e = (e_secs, h2d, d2h, note)
 
-    # max over ranks (device time), diagnostics summed over the parameter shards
+    # max over ranks (device time), units and diagnostics summed over the ranks
+    units = info["units"]
     if dist is not None:
         from paper_1907_05701_b200 import sharding
         secs = sharding.max_over_ranks(secs, dist, "cuda")
+        t_units = torch.tensor([float(units)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t_units)
+        units = float(t_units[0])
         if e2e:
             e2e = (sharding.max_over_ranks(e2e[0], dist, "cuda"),) + e2e[1:]
-        if diag is not None:
-            # the only collective: 3*S doubles, outside the timed region
+        if diag is not None and args.partition == "range" and world > 1:
+            # the only collective of the range partition: 3*S doubles, outside the timed region
             diag = sharding.allreduce_diagnostics(diag, dist, "cuda")
     arena_bytes = h.arena_bytes
+    P_rank = h.P_padded
+    S_rank = h.S
     h.close()
     del h
     torch.cuda.empty_cache()
@@ -408,12 +599,14 @@ def run_ours(args):
     # HADPSGD_SHARE_PAIR_WEIGHTS, where pair members share one weight buffer (same arithmetic and
     # results; one weight write per pair and one HBM fetch of the buffer two pairs read).
     shared = None
-    can_share = not (flags & (H.NO_MIX | H.EQ7_LITERAL | H.SHARE_PAIR_WEIGHTS)) and S > 1 and S % 2 == 0
+    can_share = (not (flags & (H.NO_MIX | H.EQ7_LITERAL | H.SHARE_PAIR_WEIGHTS)) and S > 1 and S % 2 == 0
+                 and (world == 1 or args.partition == "weak"))
     if can_share and not args.no_share_leg:
+        from fixtures import problem
         hs = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags | H.SHARE_PAIR_WEIGHTS,
                        device=local, working_dtype=H.BF16 if args.emit_bf16 else H.F32)
-        problem.fill_weights(hs, seed)
-        problem.fill_grads(hs, seed, 0, cfg["dist"])
+        problem.fill_weights(hs, 2000 + rank)
+        problem.fill_grads(hs, 2000 + rank, 0, cfg["dist"])
         torch.cuda.synchronize()
         s_secs, _ = time_device_steps(torch, dist, hs, args.steps, args.warmup)
         if dist is not None:
@@ -427,42 +620,63 @@ def run_ours(args):
     if rank == 0:
         t_step = secs / args.steps
         peak, peak_src = measured_peak()
-        abytes = algorithmic_bytes(cfg)
-        achieved = abytes / t_step / 1e9
+        per_sp = cfg["G"] * cfg["b_g"] + 16 + (2 if cfg.get("emit") else 0)        # bytes per super-learner-parameter
+        abytes_rank = S_rank * P_rank * per_sp                                      # algorithmic bytes of ONE launch (this rank)
+        achieved = abytes_rank / t_step / 1e9
+        traffic, traffic_src = (None, "n/a: per-rank launch of a partition") if world > 1 else \
+            ncu_traffic(args.workload, args.flags, args.emit_bf16)
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes_rank,
+                "kernel": "hadpsgd::step_kernel (one launch = one step)", "frac_of_8TBps_nominal": achieved / 8000.0,
+                "note": "peak is a 1:1 copy; this kernel reads more than it writes, and reads are the faster direction, "
+                        "so frac may exceed 1 (see ceiling)"}
+        if not args.no_ceiling and world == 1:
+            rd = S_rank * P_rank * (cfg["G"] * cfg["b_g"] + 8)
+            ceil = mix_ceiling(torch, rd, abytes_rank - rd)
+            ceil["frac_of_mix_ceiling"] = achieved / ceil["mix_gbs"]
+            roof["ceiling"] = ceil
         line = {
-            "metric": METRIC, "value": world * S * G * P / t_step, "unit": UNIT, "n_gpus": world,
+            "metric": METRIC, "value": units / t_step, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": info["scaling"], "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "S": S, "G": G, "P": P, "n_segments": len(cfg["seg_len"]),
                        "grad_dtype": cfg["grad"], "master_dtype": "f32",
                        "working_dtype": "bf16" if args.emit_bf16 else "f32", "lr": LR, "momentum": MU,
                        "resident_bytes_per_gpu": arena_bytes, "flags": args.flags or "default (diagnostics on)",
                        "l2": "inputs larger than L2 (working set per step >> 126 MB); no flush needed",
-                       "parallelism": "single GPU" if world == 1 else f"parameter-range shards x{world}, no data-path collective"},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None if args.emit_bf16 else NCU_TRAFFIC_BYTES.get(args.workload),
-                         "traffic_source": None if args.emit_bf16 else NCU_TRAFFIC_SOURCE.get(args.workload),
-                         "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
-                         "kernel": "hadpsgd::step_kernel (one launch = one step)", "frac_of_8TBps_nominal": achieved / 8000.0},
-            "clocks": clocks, "gpu_launches": launches,
+                       "partition": args.partition if world > 1 else "single", "parallelism": info["parallelism"]},
+            "roofline": roof, "clocks": clocks, "gpu_launches": launches,
         }
+        for k_ in ("shard", "nvlink_read_bytes_per_rank_per_step"):
+            if k_ in info:
+                line["config"][k_] = info[k_]
+        if diag is not None:
+            line["diagnostics_last_step"] = {"gsq_sum": float(diag["gsq"].sum()), "wsq_sum": float(diag["wsq"].sum()),
+                                             "gap_sum": float(diag["gap"].sum())}
         if shared is not None:
+            abytes = S * P * per_sp
             line["share_pair_weights"] = {
                 "flag": "HADPSGD_SHARE_PAIR_WEIGHTS (opt-in; bench.py --flags share makes it the headline leg)",
                 "ms_per_step": shared * 1e3, "value": world * S * G * P / shared, "unit": UNIT,
                 "achieved_algorithmic_gbs": abytes / shared / 1e9, "frac_of_peak_algorithmic": abytes / shared / 1e9 / peak,
                 "bytes_moved_model": S * P * (cfg["G"] * cfg["b_g"] + 12 + (1 if args.emit_bf16 else 0)),
-                "traffic": NCU_TRAFFIC_SHARED.get(args.workload) if not args.emit_bf16 else None,
+                "traffic": ncu_traffic(args.workload, ",".join(filter(None, [args.flags, "share"])), args.emit_bf16)[0],
                 "note": "same arithmetic and results (parity-tested at full size); pair members share one of the S weight "
                         "buffers: 4 B less written and 4 B less fetched from HBM per pair-parameter than the algorithmic "
                         "S*P*(G*b_g+16), so achieved_algorithmic_gbs exceeds the DRAM rate actually sustained"}
         if e2e:
             e_step = e2e[0] / args.e2e_steps
-            line["e2e"] = {"value": world * S * G * P / e_step, "unit": UNIT, "h2d_bytes_per_step": e2e[1],
+            h2d_gbs = e2e[1] / e_step / 1e9
+            line["e2e"] = {"value": units / e_step, "unit": UNIT, "h2d_bytes_per_step": e2e[1],
                            "d2h_bytes_per_step": e2e[2], "ms_per_step": e_step * 1e3, "steps": args.e2e_steps,
-                           "note": "hadpsgd_step_host: " + e2e[3]}
+                           "h2d_gbs": h2d_gbs, "frac_of_pcie_gen5_x16": h2d_gbs / PCIE_GEN5_X16_GBS,
+                           "note": "hadpsgd_step_host: " + e2e[3] + "; bound by the host-to-device copy of the S*G gradient "
+                                   f"buffers (PCIe Gen5 x16, {PCIE_GEN5_X16_GBS:.0f} GB/s nominal per direction), which the "
+                                   "fused kernel overlaps chunk by chunk; the new weights and momenta stay resident in HBM "
+                                   "(the learners live on the GPU), so the device-to-host traffic is the diagnostics only"}
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg, args.cpu_sample_elems, args.cpu_sample_steps)
+            line["cpu_baseline"] = cpu_baseline(cfg, args.cpu_sample_elems, args.cpu_sample_steps, args.cpu_repeats)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
@@ -472,43 +686,67 @@ def run_ours(args):
 def run_sweep(args):
     """BASELINE.json configs[4]: flat fp32 buffer of 2^10..2^28 params (powers of 4), G in {2,4,8},
     S in {2,4,8,16} with S*G*P*4 B <= 96 GB; uniform grads in [-1e-3, 1e-3]; W warm + K timed steps
-    per point (defaults 5 + 20); GB/s (algorithmic) vs buffer size.  Small points are L2-resident
-    (working set < 126 MB) and launch-latency bound: they are flagged, not bandwidth claims."""
+    per point (defaults 5 + 20); GB/s (algorithmic) vs buffer size.  Every point is timed twice: the K
+    steps enqueued one by one from Python ("eager": below ~10 us per step this measures the host's launch
+    path, not the GPU), and the same K steps captured once into a CUDA graph and replayed (what a
+    launch-bound caller does; hadpsgd_step only enqueues, so it captures).  Small points are L2-resident
+    (working set < 126 MB) and latency-bound: they are flagged, not bandwidth claims."""
     import torch
     import paper_1907_05701_b200 as H
     from fixtures import problem, shapes
     H.lib()
     torch.cuda.set_device(0)
     peak, peak_src = measured_peak()
+    side = torch.cuda.Stream()
     rows = []
     for P, S, G in shapes.sweep_points():
-        h = H.Hadpsgd(S, G, [P], H.F32, parse_flags(H, args.flags), device=0)
-        problem.fill_weights(h, 3000)
-        problem.fill_grads(h, 3000, 0, "uniform")
-        torch.cuda.synchronize()
-        secs, _ = time_device_steps(torch, None, h, args.steps, args.warmup)
-        t = secs / args.steps
+        if P > (1 << args.sweep_max_log2):
+            continue
+        with torch.cuda.stream(side):
+            h = H.Hadpsgd(S, G, [P], H.F32, parse_flags(H, args.flags), device=0, stream=side)
+            problem.fill_weights(h, 3000)
+            problem.fill_grads(h, 3000, 0, "uniform")
+            torch.cuda.synchronize()
+            secs, _ = time_device_steps(torch, None, h, args.steps, args.warmup)
+            t_eager = secs / args.steps
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                for k in range(args.steps):
+                    h.hadpsgd_step(LR, MU, k)
+            for _ in range(max(1, args.warmup // 2)):
+                graph.replay()
+            torch.cuda.synchronize()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record(side)
+            graph.replay()
+            ev1.record(side)
+            torch.cuda.synchronize()
+            t_graph = ev0.elapsed_time(ev1) / 1e3 / args.steps
+        t = min(t_eager, t_graph)
         cfg = {"S": S, "G": G, "P": P, "b_g": 4}
-        row = {"P": P, "S": S, "G": G, "us_per_step": t * 1e6, "gb_per_s": algorithmic_bytes(cfg) / t / 1e9,
+        row = {"P": P, "S": S, "G": G, "us_per_step": t * 1e6, "us_per_step_eager": t_eager * 1e6,
+               "us_per_step_graph": t_graph * 1e6, "gb_per_s": algorithmic_bytes(cfg) / t / 1e9,
                "learner_params_per_s": S * G * P / t, "resident_bytes": h.arena_bytes,
                "l2_resident": h.arena_bytes < 126e6}
         row["frac_of_measured_peak"] = row["gb_per_s"] / peak
         rows.append(row)
         print(json.dumps(row), flush=True)
         h.close()
-        del h
+        del h, graph
         torch.cuda.empty_cache()
     if args.sweep_md:
         with open(args.sweep_md, "w") as f:
             f.write(f"# Bandwidth sweep (BASELINE.json configs[4])\n\nCommand: `python bench.py --sweep --steps {args.steps} "
                     f"--warmup {args.warmup} --sweep-md {args.sweep_md}`; flat fp32, uniform gradients, diagnostics on; "
-                    f"GB/s = S*P*(4G+16) / t_step; peak = {peak} GB/s ({peak_src}).  Points whose resident set is below the "
-                    "126 MB L2 are marked L2: their GB/s is cache bandwidth or launch latency, not HBM.\n\n")
-            f.write("| P | S | G | resident MB | us/step | GB/s | of peak | |\n|---|---|---|---|---|---|---|---|\n")
+                    f"each point: {args.steps} steps enqueued from Python (eager) and the same {args.steps} steps as one CUDA-graph "
+                    f"replay; us/step = the faster of the two; GB/s = S*P*(4G+16) / t_step; peak = {peak} GB/s ({peak_src}).  "
+                    "Points whose resident set is below the 126 MB L2 are marked L2: their GB/s is cache bandwidth or launch "
+                    "latency, not HBM.\n\n")
+            f.write("| P | S | G | resident MB | us/step eager | us/step graph | GB/s | of peak | |\n|---|---|---|---|---|---|---|---|---|\n")
             for r in rows:
                 f.write(f"| 2^{r['P'].bit_length() - 1} | {r['S']} | {r['G']} | {r['resident_bytes'] / 1e6:.1f} | "
-                        f"{r['us_per_step']:.2f} | {r['gb_per_s']:.1f} | {r['frac_of_measured_peak']:.3f} | "
-                        f"{'L2' if r['l2_resident'] else ''} |\n")
+                        f"{r['us_per_step_eager']:.2f} | {r['us_per_step_graph']:.2f} | {r['gb_per_s']:.1f} | "
+                        f"{r['frac_of_measured_peak']:.3f} | {'L2' if r['l2_resident'] else ''} |\n")
 
 
 def main():

@@ -11,16 +11,18 @@ from . import generator as gen
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "gen_device.cu")
+SRC_MEMBENCH = os.path.join(HERE, "membench.cu")
 LIB = os.path.join(HERE, "libhadpsgd_fixture.so")
 _lib = None
 
 
 def build(force=False):
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    newest = max(os.path.getmtime(SRC), os.path.getmtime(SRC_MEMBENCH))
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--ftz=false",
-                    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", LIB, SRC], check=True)
+                    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", LIB, SRC, SRC_MEMBENCH], check=True)
     return LIB
 
 
@@ -30,8 +32,35 @@ def lib():
         L = ctypes.CDLL(build())
         L.hadpsgd_fixture_fill.argtypes = [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_longlong, ctypes.c_uint64,
                                            ctypes.c_float, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
+        L.hadpsgd_fixture_membench.argtypes = [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_int,
+                                               ctypes.c_void_p, ctypes.c_void_p]
         _lib = L
     return _lib
+
+
+def membench(total_bytes=8 << 30, n_streams=12, write=False, reps=5):
+    """This device's streaming rate in GB/s (best of `reps`), read or write, n_streams buffers walked in
+    lock step with the step kernel's access shape (fixtures/membench.cu)."""
+    import torch
+    stream_bytes = total_bytes // n_streams // 8192 * 8192
+    buf = torch.empty(stream_bytes * n_streams + 256, dtype=torch.uint8, device="cuda")
+    if not write:
+        buf.random_(0, 255)
+    sink = buf[stream_bytes * n_streams:]
+    st = torch.cuda.current_stream().cuda_stream
+    best = 0.0
+    for i in range(reps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        rc = lib().hadpsgd_fixture_membench(buf.data_ptr(), stream_bytes, n_streams, 1 if write else 0, sink.data_ptr(), st)
+        if rc != 0:
+            raise RuntimeError(f"membench launch failed: cudaError {rc}")
+        e1.record()
+        torch.cuda.synchronize()
+        if i:                                   # the first pass is a warm-up
+            best = max(best, stream_bytes * n_streams / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    del buf
+    return best
 
 
 def fill(tensor, key, dist="normal", scale=1e-3, elem_offset=0, n=None, stream=None):

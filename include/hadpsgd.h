@@ -58,12 +58,16 @@ enum { /* hadpsgd_opts.flags */
     HADPSGD_NO_MIX        = 1u << 1, /* T_k = I: eq. (6)/(3) only, every super-learner keeps u_s         */
     HADPSGD_NO_DIAG       = 1u << 2, /* skip a5                                                          */
     HADPSGD_EQ7_LITERAL   = 1u << 3, /* eq. (7) as printed: w'_s = 1/2 (w_s + w_p) - lr v_s  (row f1)    */
-    HADPSGD_SHARE_PAIR_WEIGHTS = 1u << 4 /* both members of a pair end a step with identical weights (R3),
+    HADPSGD_SHARE_PAIR_WEIGHTS = 1u << 4, /* both members of a pair end a step with identical weights (R3),
                                         so they SHARE one of the S weight buffers: one weight write per
                                         pair instead of two, and the buffer two neighbouring pairs read
                                         next step is fetched from HBM once.  Same arithmetic, same
                                         results; what changes is which buffer hadpsgd_weights(h, s)
                                         points to (see there).  Not with NO_MIX or EQ7_LITERAL.          */
+    HADPSGD_PEER = 1u << 5           /* this handle holds the super-learners of ONE rank of a super-learner
+                                        partition (row f4): see "super-learner partition"
+                                        below.  Needs dtypes.peer_stage = 1.  Not with EQ7_LITERAL,
+                                        SHARE_PAIR_WEIGHTS or a bf16 working copy.                        */
 };
 
 #define HADPSGD_SEG_ALIGN_ELEMS 64 /* 256 B in fp32, 128 B in bf16 */
@@ -76,13 +80,16 @@ typedef struct {
                              extra is stored.  HADPSGD_BF16: every step ALSO writes a bf16
                              (round-to-nearest-even) copy of each new weight buffer for
                              mixed-precision learners (+2 B per parameter per super-learner; row f2) */
+    int32_t peer_stage;   /* 0 (default) | 1: also lay out two fp32 STAGE buffers per super-learner behind
+                             the S weight buffers (+8 B per parameter per super-learner), in which the
+                             halves of a mix between two arenas wait; required by HADPSGD_PEER          */
 } hadpsgd_dtypes;
 
 typedef struct {
     void*    arena;       /* dev; optional caller-owned memory (e.g. a torch uint8 tensor), 256 B aligned */
     size_t   arena_bytes; /* >= hadpsgd_required_bytes()                                                   */
     void*    stream;      /* cudaStream_t; NULL = the legacy default stream                                */
-    uint32_t flags;       /* HADPSGD_DETERMINISTIC | NO_MIX | NO_DIAG | EQ7_LITERAL                        */
+    uint32_t flags;       /* HADPSGD_DETERMINISTIC | NO_MIX | NO_DIAG | EQ7_LITERAL | SHARE_PAIR_WEIGHTS | PEER */
     int32_t  device;      /* CUDA device ordinal; -1 = current device                                      */
 } hadpsgd_opts;
 
@@ -92,7 +99,15 @@ typedef struct { /* host-side copy of the a5 diagnostics of the most recent step
     uint64_t step_k;
     double   gsq[HADPSGD_MAX_S]; /* sum_i gbar_s[i]^2                                  */
     double   wsq[HADPSGD_MAX_S]; /* sum_i w'_s[i]^2                                    */
-    double   gap[HADPSGD_MAX_S]; /* sum_i (u_s[i]-u_p[i])^2 ; gap[s]==gap[p]; 0 if unpaired */
+    double   gap[HADPSGD_MAX_S]; /* sum_i (a_s[i]-a_p[i])^2 over the two vectors the mix averages (u; the old
+                                    w under EQ7_LITERAL); gap[s]==gap[p]; exactly 0 if unmixed (R14) */
+    /* HADPSGD_PEER only (all zero otherwise).  A member whose partner lives in another arena cannot
+     * finish its mix inside this step: it reports wsq[s] = sum u_s^2, gap[s] = 0 and pending[s] = 1.
+     * The launch that resolves the mix (the next step, or hadpsgd_peer_flush) then delivers what that
+     * step still owed: pend_wsq[s] = sum_i w'_s[i]^2 and pend_gap[s] = sum_i (u_s[i]-u_p[i])^2.       */
+    double   pend_wsq[HADPSGD_MAX_S];
+    double   pend_gap[HADPSGD_MAX_S];
+    int32_t  pending[HADPSGD_MAX_S]; /* after the most recent step: 1 = the mix of s awaits its partner   */
 } hadpsgd_diag;
 
 /* a0 replica allocator (host only, no GPU needed) ------------------------------------------- */
@@ -107,7 +122,8 @@ int hadpsgd_required_bytes(int S, int G, const int64_t* seg_len /*host [n_seg]*/
  * weight buffer s   = arena + w_off + s * P_padded * 4
  * momentum buffer s = arena + v_off + s * P_padded * 4
  * gradient (s,g)    = arena + g_off + (s*G + g) * P_padded * sizeof(grad_dtype)
- * bf16 working copy s = arena + wb_off + s * P_padded * 2   (only with working_dtype == BF16)  */
+ * bf16 working copy s = arena + wb_off + s * P_padded * 2   (only with working_dtype == BF16)
+ * stage buffer (e, s) = arena + w_off + (S*(1+e) + s) * P_padded * 4   (only with peer_stage == 1)   */
 int hadpsgd_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtypes dt,
                    int64_t* seg_offset, int64_t* P_padded,
                    size_t* w_off, size_t* v_off, size_t* g_off, size_t* wb_off);
@@ -195,12 +211,60 @@ int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out);
  * synchronises the stream.  D_out: host.  Identity: D(u) - D(w') = 1/2 sum_pairs gap.         */
 int hadpsgd_consensus(hadpsgd_handle h, double* D_out);
 
+/* super-learner partition (row f4; Fig. 3) -------------------------------------
+ * The paper's topology: every node holds ONE super-learner group and exchanges weights with its ring
+ * neighbours.  Here `world` handles ("ranks": one per GPU and process, or several on one device),
+ * each created with HADPSGD_PEER and dtypes.peer_stage = 1 over the same segment table, together hold
+ * S_global super-learners: rank r owns the global indices [rank_begin[r], rank_begin[r+1]) and S of
+ * its hadpsgd_create() call must equal that count.  hadpsgd_step() then uses the ring matching on
+ * S_global, and hadpsgd_step_matching() takes partner[S_global].
+ *   A pair whose members both live in this handle is mixed as usual.  A member whose partner lives in
+ * another handle writes its u = w - lr v' into a STAGE buffer instead (stage parity = epoch & 1) and
+ * its mix stays PENDING; the next launch of BOTH owners forms w = 1/2 (u_own + u_partner) on the fly,
+ * reading the partner's stage buffer through a peer pointer inside the same fused pass -- 4 B per
+ * parameter per pending member cross the link per step, and no kernel ever waits on another one.
+ * Same arithmetic as the single-arena step: bit-exact in DETERMINISTIC mode.
+ *   Contract: (1) every rank makes the same sequence of step calls (like a collective); each call
+ * advances the handle's epoch; (2) EPOCH BARRIER -- a rank must not enqueue epoch e+1 before every
+ * rank's epoch-e kernel has completed: one stream when the handles share a device, else a
+ * stream-ordered barrier between steps (e.g. an NCCL all-reduce of one element on the handle's
+ * stream); (3) hadpsgd_weights(h, s) is INVALID_ARG while s is pending -- call hadpsgd_peer_flush()
+ * (after the epoch barrier) to materialise every pending mix into the main weight buffers.       */
+
+/* rank_begin: host [world+1], increasing, rank_begin[0] = 0, rank_begin[world] = S_global <= HADPSGD_MAX_S. */
+int hadpsgd_peer_init(hadpsgd_handle h, int rank, int world, const int32_t* rank_begin);
+/* This handle's stage region: dev pointer to [2][S][P_padded] floats (stage parity, local member). */
+int hadpsgd_peer_stage(hadpsgd_handle h, float** dev_ptr);
+/* Tell this handle where rank r's stage region is: a dev pointer VALID IN THIS PROCESS AND ON THIS
+ * DEVICE'S KERNELS (the same device, or a peer device with access enabled by the caller).  Every
+ * rank other than the handle's own must be attached before the first step.                       */
+int hadpsgd_peer_attach(hadpsgd_handle h, int r, const float* stage_region_of_rank_r);
+/* Across processes: export this handle's arena as a CUDA IPC handle (ipc_handle_out: host, 64 bytes)
+ * plus the byte offset of the stage region from the exported allocation's base ...                 */
+int hadpsgd_peer_ipc_export(hadpsgd_handle h, void* ipc_handle_out, uint64_t* stage_offset_out);
+/* ... and open rank r's export in this process (cudaIpcOpenMemHandle with lazy peer access), then
+ * attach it.  The mapping is closed by hadpsgd_destroy().                                           */
+int hadpsgd_peer_ipc_attach(hadpsgd_handle h, int r, const void* ipc_handle, uint64_t stage_offset);
+/* Materialise every pending mix: w_s = 1/2 (u_own + u_partner) into the main weight buffer (one small
+ * kernel on the stream; asynchronous), delivering pend_wsq / pend_gap.  Call after the epoch barrier.
+ * Not a step: the epoch does not advance, ranks need not call it together.                          */
+int hadpsgd_peer_flush(hadpsgd_handle h);
+/* The peer plan of one step as a pure host function (no GPU): see csrc/scheduler.cpp.  pending: in/out
+ * [S_local] (global partner index or -1); outputs [S_local]: kind (0 pair member, 1 unmixed,
+ * 2 straddling), mate (local pair mate or -1), read_buf / write_buf (weight buffer index: main s,
+ * stage (e, s) = S_local (1 + e) + s), read_peer (-1 or e * S_global + global partner).           */
+int hadpsgd_plan_peer(int world, int rank, const int32_t* rank_begin, const int32_t* partner /*[S_global]*/,
+                      uint64_t epoch, int32_t* pending, int32_t* kind, int32_t* mate, int32_t* read_buf,
+                      int32_t* write_buf, int32_t* read_peer);
+
 /* Measurement knob: resident blocks per SM of the persistent grid (1..16, clamped to what fits);
  * 0 restores the default chosen per (G, dtype, mode).  Results do not depend on it.          */
 int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm);
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int hadpsgd_launch_count(hadpsgd_handle h, uint64_t* out);
 
+/* Thread safety: the pure host functions above are re-entrant.  A handle is NOT thread-safe: calls on
+ * one handle must be serialised by the caller; different handles may be used from different threads. */
 const char* hadpsgd_error_string(int code);
 const char* hadpsgd_last_error(hadpsgd_handle h);
 

@@ -11,7 +11,7 @@ import numpy as np
 
 F32, BF16 = 0, 1
 OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_DEVICE = 0, -1, -2, -3, -4
-DETERMINISTIC, NO_MIX, NO_DIAG, EQ7_LITERAL, SHARE_PAIR_WEIGHTS = 1, 2, 4, 8, 16
+DETERMINISTIC, NO_MIX, NO_DIAG, EQ7_LITERAL, SHARE_PAIR_WEIGHTS, PEER = 1, 2, 4, 8, 16, 32
 SEG_ALIGN_ELEMS = 64
 MAX_S = 512
 
@@ -20,7 +20,8 @@ LIB_PATH = os.path.join(_HERE, "libhadpsgd.so")
 
 
 class hadpsgd_dtypes(ctypes.Structure):
-    _fields_ = [("grad_dtype", ctypes.c_int32), ("master_dtype", ctypes.c_int32), ("working_dtype", ctypes.c_int32)]
+    _fields_ = [("grad_dtype", ctypes.c_int32), ("master_dtype", ctypes.c_int32), ("working_dtype", ctypes.c_int32),
+                ("peer_stage", ctypes.c_int32)]
 
 
 class hadpsgd_opts(ctypes.Structure):
@@ -30,7 +31,9 @@ class hadpsgd_opts(ctypes.Structure):
 
 class hadpsgd_diag(ctypes.Structure):
     _fields_ = [("S", ctypes.c_int32), ("n_pairs", ctypes.c_int32), ("step_k", ctypes.c_uint64),
-                ("gsq", ctypes.c_double * MAX_S), ("wsq", ctypes.c_double * MAX_S), ("gap", ctypes.c_double * MAX_S)]
+                ("gsq", ctypes.c_double * MAX_S), ("wsq", ctypes.c_double * MAX_S), ("gap", ctypes.c_double * MAX_S),
+                ("pend_wsq", ctypes.c_double * MAX_S), ("pend_gap", ctypes.c_double * MAX_S),
+                ("pending", ctypes.c_int32 * MAX_S)]
 
 
 class HadpsgdError(RuntimeError):
@@ -74,6 +77,13 @@ def lib():
         L.hadpsgd_unshare.argtypes = [vp]
         L.hadpsgd_plan_slots.argtypes = [i32, i32p, i32, i32p, i32p, i32p, i32p, i32p, i32p]
         L.hadpsgd_consensus.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        L.hadpsgd_peer_init.argtypes = [vp, i32, i32, i32p]
+        L.hadpsgd_peer_stage.argtypes = [vp, ctypes.POINTER(vp)]
+        L.hadpsgd_peer_attach.argtypes = [vp, i32, vp]
+        L.hadpsgd_peer_ipc_export.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_uint64)]
+        L.hadpsgd_peer_ipc_attach.argtypes = [vp, i32, vp, ctypes.c_uint64]
+        L.hadpsgd_peer_flush.argtypes = [vp]
+        L.hadpsgd_plan_peer.argtypes = [i32, i32, i32p, i32p, u64, i32p, i32p, i32p, i32p, i32p, i32p]
         L.hadpsgd_set_launch.argtypes = [vp, i32]
         L.hadpsgd_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.hadpsgd_error_string.argtypes = [i32]
@@ -96,19 +106,20 @@ def _check(rc, h=None):
         raise HadpsgdError(rc, f"{L.hadpsgd_error_string(rc).decode()}: {detail}")
 
 
-def hadpsgd_required_bytes(S, G, seg_len, grad_dtype=F32, working_dtype=F32):
+def hadpsgd_required_bytes(S, G, seg_len, grad_dtype=F32, working_dtype=F32, peer_stage=0):
     arr, n = _seg(seg_len)
     out = ctypes.c_size_t(0)
-    _check(lib().hadpsgd_required_bytes(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype), ctypes.byref(out)))
+    _check(lib().hadpsgd_required_bytes(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype, peer_stage),
+                                        ctypes.byref(out)))
     return out.value
 
 
-def hadpsgd_layout(S, G, seg_len, grad_dtype=F32, working_dtype=F32):
+def hadpsgd_layout(S, G, seg_len, grad_dtype=F32, working_dtype=F32, peer_stage=0):
     arr, n = _seg(seg_len)
     seg_off = (ctypes.c_int64 * n)()
     P = ctypes.c_int64(0)
     w, v, g, wb = ctypes.c_size_t(0), ctypes.c_size_t(0), ctypes.c_size_t(0), ctypes.c_size_t(0)
-    _check(lib().hadpsgd_layout(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype), seg_off, ctypes.byref(P),
+    _check(lib().hadpsgd_layout(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype, peer_stage), seg_off, ctypes.byref(P),
                                 ctypes.byref(w), ctypes.byref(v), ctypes.byref(g), ctypes.byref(wb)))
     return dict(seg_offset=list(seg_off), P_padded=P.value, w_off=w.value, v_off=v.value, g_off=g.value,
                 wb_off=wb.value)
@@ -142,12 +153,31 @@ def hadpsgd_plan_slots(partner, w_slot, share=True):
     return list(ws), list(rd), list(wr), [(cs[i], cd[i]) for i in range(n.value)]
 
 
+def hadpsgd_plan_peer(world, rank, rank_begin, partner, epoch, pending):
+    """Pure host function: the peer plan of one step for `rank` (see include/hadpsgd.h).  Returns a dict
+    of lists indexed by the LOCAL member: pending (after the step), kind, mate, read_buf, write_buf,
+    read_peer."""
+    ok = 0 <= rank < world and len(rank_begin) == world + 1
+    S_l = max(rank_begin[rank + 1] - rank_begin[rank], 1) if ok else 1      # the library rejects bad ranks
+    if len(rank_begin) != world + 1:
+        raise HadpsgdError(INVALID_ARG, "rank_begin must have world + 1 entries")
+    i32a = lambda v: (ctypes.c_int32 * len(v))(*[int(x) for x in v])
+    rb, pt, pend = i32a(rank_begin), i32a(partner), i32a(pending)
+    outs = [i32a([0] * S_l) for _ in range(5)]
+    _check(lib().hadpsgd_plan_peer(world, rank, rb, pt, epoch, pend, *outs))
+    names = ("kind", "mate", "read_buf", "write_buf", "read_peer")
+    d = {n: list(o) for n, o in zip(names, outs)}
+    d["pending"] = list(pend)
+    return d
+
+
 class Hadpsgd:
     """Handle wrapper.  Device memory is a torch uint8 tensor (the arena) so that torch owns
     allocation and stream plumbing; everything else happens behind the C ABI."""
 
     def __init__(self, S, G, seg_len, grad_dtype=F32, flags=0, device=0, stream=None, own_arena=False,
                  working_dtype=F32):
+        peer_stage = 1 if flags & PEER else 0
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("hadpsgd needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -156,8 +186,8 @@ class Hadpsgd:
         self.torch = torch
         self.device = torch.device("cuda", device)
         arr, n = _seg(self.seg_len)
-        nbytes = hadpsgd_required_bytes(S, G, self.seg_len, grad_dtype, working_dtype)
-        self.layout = hadpsgd_layout(S, G, self.seg_len, grad_dtype, working_dtype)
+        nbytes = hadpsgd_required_bytes(S, G, self.seg_len, grad_dtype, working_dtype, peer_stage)
+        self.layout = hadpsgd_layout(S, G, self.seg_len, grad_dtype, working_dtype, peer_stage)
         self.P_padded = self.layout["P_padded"]
         opts = hadpsgd_opts()
         opts.flags, opts.device = flags, device
@@ -172,7 +202,7 @@ class Hadpsgd:
         self.arena_bytes = nbytes
         h = ctypes.c_void_p()
         with torch.cuda.device(self.device):
-            _check(lib().hadpsgd_create(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype), ctypes.byref(opts),
+            _check(lib().hadpsgd_create(S, G, arr, n, hadpsgd_dtypes(grad_dtype, F32, working_dtype, peer_stage), ctypes.byref(opts),
                                         ctypes.byref(h)))
         self.h = h
 
@@ -181,7 +211,7 @@ class Hadpsgd:
         _check(lib().hadpsgd_step(self.h, lr, momentum, step_k), self.h)
 
     def hadpsgd_step_matching(self, lr, momentum, step_k, partner):
-        arr = (ctypes.c_int32 * self.S)(*[int(p) for p in partner])
+        arr = (ctypes.c_int32 * len(partner))(*[int(p) for p in partner])   # S entries (S_global in peer mode)
         _check(lib().hadpsgd_step_matching(self.h, lr, momentum, step_k, arr), self.h)
 
     def hadpsgd_step_host(self, host_grad_ptrs, lr, momentum, step_k, want_diag=True):
@@ -238,7 +268,8 @@ class Hadpsgd:
     def _diag_dict(self, d):
         S = d.S
         return dict(step_k=d.step_k, n_pairs=d.n_pairs, gsq=np.array(d.gsq[:S]), wsq=np.array(d.wsq[:S]),
-                    gap=np.array(d.gap[:S]))
+                    gap=np.array(d.gap[:S]), pend_wsq=np.array(d.pend_wsq[:S]), pend_gap=np.array(d.pend_gap[:S]),
+                    pending=np.array(d.pending[:S]))
 
     def hadpsgd_diagnostics(self):
         d = hadpsgd_diag()
@@ -252,6 +283,32 @@ class Hadpsgd:
         out = ctypes.c_double(0.0)
         _check(lib().hadpsgd_consensus(self.h, ctypes.byref(out)), self.h)
         return out.value
+
+    # -- super-learner partition (HADPSGD_PEER) ------------------------------------------
+    def hadpsgd_peer_init(self, rank, world, rank_begin):
+        arr = (ctypes.c_int32 * (world + 1))(*[int(x) for x in rank_begin])
+        _check(lib().hadpsgd_peer_init(self.h, rank, world, arr), self.h)
+
+    def hadpsgd_peer_stage(self):
+        p = ctypes.c_void_p()
+        _check(lib().hadpsgd_peer_stage(self.h, ctypes.byref(p)), self.h)
+        return p.value
+
+    def hadpsgd_peer_attach(self, r, stage_ptr):
+        _check(lib().hadpsgd_peer_attach(self.h, r, ctypes.c_void_p(stage_ptr)), self.h)
+
+    def hadpsgd_peer_ipc_export(self):
+        buf = ctypes.create_string_buffer(64)
+        off = ctypes.c_uint64(0)
+        _check(lib().hadpsgd_peer_ipc_export(self.h, buf, ctypes.byref(off)), self.h)
+        return bytes(buf.raw), off.value
+
+    def hadpsgd_peer_ipc_attach(self, r, ipc_bytes, stage_offset):
+        buf = ctypes.create_string_buffer(ipc_bytes, 64)
+        _check(lib().hadpsgd_peer_ipc_attach(self.h, r, buf, stage_offset), self.h)
+
+    def hadpsgd_peer_flush(self):
+        _check(lib().hadpsgd_peer_flush(self.h), self.h)
 
     def hadpsgd_set_launch(self, blocks_per_sm=0):
         _check(lib().hadpsgd_set_launch(self.h, blocks_per_sm), self.h)

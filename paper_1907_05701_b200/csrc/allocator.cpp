@@ -6,7 +6,8 @@
 // north_star (a)).  One weight + one momentum copy per SUPER-learner: the G learners of a
 // super-learner have staleness 0, so their replicas are identical and are
 // collapsed (R18).  With dtypes.working_dtype == BF16 a fourth region holds S bf16
-// working copies of the weights (row f2).
+// working copies of the weights (row f2).  With dtypes.peer_stage the weight region also holds two
+// stage buffers per super-learner, in which the halves of a mix between two arenas wait (row f4).
 #include "internal.h"
 
 namespace hadpsgd {
@@ -23,9 +24,12 @@ int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
     if (dt.grad_dtype != HADPSGD_F32 && dt.grad_dtype != HADPSGD_BF16) return fail("grad_dtype must be F32 or BF16");
     if (dt.master_dtype != HADPSGD_F32) return fail("master_dtype must be F32");
     if (dt.working_dtype != HADPSGD_F32 && dt.working_dtype != HADPSGD_BF16) return fail("working_dtype must be F32 (none) or BF16");
+    if (dt.peer_stage != 0 && dt.peer_stage != 1) return fail("peer_stage must be 0 or 1");
+    if (dt.peer_stage && dt.working_dtype != HADPSGD_F32) return fail("peer_stage (HADPSGD_PEER) has no bf16 working copy");
 
     Layout L;
     L.S = S; L.G = G; L.n_seg = n_seg; L.grad_dtype = dt.grad_dtype; L.working_dtype = dt.working_dtype;
+    L.peer_stage = dt.peer_stage;
     L.seg_len.assign(seg_len, seg_len + n_seg);
     L.seg_offset.resize(n_seg);
     int64_t off = 0;
@@ -40,15 +44,20 @@ int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
     L.P_padded = off;
 
     size_t cur = 0;
-    L.w_off = cur; cur = round_up(cur + static_cast<size_t>(S) * L.w_stride_bytes(), kRegionAlign);
+    // weights: S main buffers, then (peer_stage) 2 x S stage buffers, contiguous: buffer x = w_off + x * P * 4
+    L.w_off = cur;
+    L.stage_off = cur + static_cast<size_t>(S) * L.w_stride_bytes();
+    cur = round_up(cur + static_cast<size_t>(S) * (L.peer_stage ? 3 : 1) * L.w_stride_bytes(), kRegionAlign);
     L.v_off = cur; cur = round_up(cur + static_cast<size_t>(S) * L.w_stride_bytes(), kRegionAlign);
     L.g_off = cur; cur = round_up(cur + static_cast<size_t>(S) * G * L.g_stride_bytes(), kRegionAlign);
     L.wb_off = cur;
     if (L.working_dtype == HADPSGD_BF16) cur = round_up(cur + static_cast<size_t>(S) * L.P_padded * 2, kRegionAlign);
-    // aux: per-block partial sums [S items][5][kMaxGridBlocks] doubles, results [3*S] doubles, ticket
+    // aux: per-block partial sums [kMaxGridBlocks][items per launch x quantities] doubles, the results
+    // (kDiagArrays x S doubles), the ticket
+    const int items = S < kMaxItemsPerLaunch ? S : kMaxItemsPerLaunch;
     L.aux_off = cur;
-    L.aux_bytes = round_up(static_cast<size_t>(S) * kDiagQuantities * kMaxGridBlocks * sizeof(double) +
-                           static_cast<size_t>(3 * S) * sizeof(double) + 256, kRegionAlign);
+    L.aux_bytes = round_up(static_cast<size_t>(items) * kMaxDiagQuantities * kMaxGridBlocks * sizeof(double) +
+                           static_cast<size_t>(kDiagArrays * S) * sizeof(double) + 256, kRegionAlign);
     cur += L.aux_bytes;
     L.total_bytes = cur;
     *out = L;

@@ -13,6 +13,9 @@
 
 using namespace hadpsgd;
 
+// The launches of one step: pair items, then unmixed / publishing single items.
+struct StepPlan { std::vector<WorkItem> pairs, singles; bool shared = false; };
+
 struct hadpsgd_ctx {
     Layout L;
     uint32_t flags = 0;
@@ -22,7 +25,6 @@ struct hadpsgd_ctx {
     cudaStream_t copy_stream = nullptr;   // host path: H2D copies overlap the kernel
     std::vector<cudaEvent_t> chunk_events;
     std::vector<std::pair<const void*, int>> occupancy;   // per kernel instantiation, queried once
-    std::vector<std::pair<const void*, size_t>> smem_optin; // largest dynamic smem opted in per kernel
     std::vector<int32_t> w_slot;                           // slot (buffer index) that holds w_s right now
     char* arena = nullptr;
     bool owns_arena = false;
@@ -33,6 +35,17 @@ struct hadpsgd_ctx {
     int last_n_pairs = 0;
     uint64_t launches = 0;
     int blocks_per_sm = 0;   // tuning override of the persistent grid (0 = the plan's default)
+    std::vector<int32_t> partner;   // scratch of the step calls (no allocation per step)
+    StepPlan plan;
+    // super-learner partition (HADPSGD_PEER)
+    bool peer_init = false, peer_table_dirty = true;
+    int rank = 0, world = 1, S_global = 0;
+    std::vector<int32_t> rank_begin;
+    std::vector<const float*> stage_of_rank;   // [world] stage regions as seen from this process
+    std::vector<int32_t> pending;              // [S] global partner whose stage completes w_s, or -1
+    uint64_t epoch = 0;
+    const float** d_peer = nullptr;            // device table [2][S_global]
+    std::vector<void*> ipc_mapped;             // cudaIpcOpenMemHandle results, closed at destroy
     std::string err;
 };
 
@@ -46,6 +59,14 @@ static thread_local std::string g_create_error;
             return HADPSGD_CUDA;                                                            \
         }                                                                                   \
     } while (0)
+
+namespace hadpsgd {
+int launch_consensus(const float* w, long long P_padded, int S, const int32_t* w_slot, int num_sms,
+                     double* block_out, cudaStream_t stream, cudaError_t* err);   // consensus.cu
+int launch_peer_flush(float* w_main, const float* a_stage, const float* const* peer, const int32_t* members,
+                      int n_members, long long P_padded, int S, int num_sms, double* partials, double* diag,
+                      bool exact, cudaStream_t stream, cudaError_t* err);         // peer_flush.cu
+}
 
 // ---- kernel dispatch -------------------------------------------------------------------
 namespace {
@@ -63,15 +84,18 @@ struct DeviceGuard {
     DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
+bool is_peer(const hadpsgd_ctx* h) { return (h->flags & HADPSGD_PEER) != 0; }
+
 int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, bool shared_slots, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
     const bool exact = h->flags & HADPSGD_DETERMINISTIC;
     const bool diag = !(h->flags & HADPSGD_NO_DIAG);
     const bool emit = h->L.working_dtype == HADPSGD_BF16;
-    const bool shared = shared_slots && mode == kPair;   // pair members share weight slots
-    LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode, shared) : plan_f32_emit(h->L.G, exact, diag, mode, shared))
-                           : (bf16 ? plan_bf16(h->L.G, exact, diag, mode, shared) : plan_f32(h->L.G, exact, diag, mode, shared));
+    const int wmode = is_peer(h) ? kPeer : ((shared_slots && mode == kPair) ? kSlots : kOwn);
+    LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode, wmode) : plan_f32_emit(h->L.G, exact, diag, mode, wmode))
+                           : (bf16 ? plan_bf16(h->L.G, exact, diag, mode, wmode) : plan_f32(h->L.G, exact, diag, mode, wmode));
+    if (!plan.fn) { h->err = "this combination of flags has no kernel"; return HADPSGD_INVALID_ARG; }
 
     const int unit = bf16 ? 16 : 8;   // elements per 32-byte gradient vector
     StepArgs a;
@@ -79,6 +103,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
     a.v = reinterpret_cast<float*>(h->arena + h->L.v_off);
     a.g = h->arena + h->L.g_off;
     a.wb = emit ? h->arena + h->L.wb_off : nullptr;
+    a.peer = h->d_peer;
     a.P = h->L.P_padded;
     a.unit_begin = elem_begin / unit;
     a.unit_end = elem_end / unit;
@@ -87,27 +112,33 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
     a.lr = lr; a.mu = mu;
     a.invG = 1.0f / static_cast<float>(h->L.G);   // fp32 reciprocal, exact for G = 1,2,4,8 (R5)
     a.accumulate_diag = accumulate ? 1 : 0;
+    a.tile_major = wmode == kSlots ? 1 : 0;
     a.S = h->L.S;
     a.partials = h->d_partials; a.diag = h->d_diag; a.ticket = h->d_ticket;
-    for (int j = 0; j < n_items; ++j)
-        a.work[j] = pack_item(items[j].s, items[j].p, items[j].ws, items[j].wp, items[j].wo_s, items[j].wo_p);
+    for (int j = 0; j < n_items; ++j) {
+        const WorkItem& it = items[j];
+        a.items[j] = {static_cast<unsigned short>(it.s), static_cast<unsigned short>(it.p),
+                      static_cast<unsigned short>(it.ws), static_cast<unsigned short>(it.wp),
+                      static_cast<unsigned short>(it.wo_s), static_cast<unsigned short>(it.wo_p),
+                      static_cast<unsigned short>(it.b_s), static_cast<unsigned short>(it.b_p)};
+    }
 
+    // per-warp diagnostic accumulators [warps][items][quantities]; the last block's column sums reuse
+    // the buffer and need max(threads, rows) doubles.  At most 18 KB: no opt-in needed.
+    const int nq = wmode == kPeer ? kNQPeer : kNQ;
+    size_t smem = 0;
+    if (diag) {
+        size_t cells = static_cast<size_t>(plan.threads / 32) * n_items * nq;
+        if (cells < static_cast<size_t>(plan.threads)) cells = plan.threads;
+        smem = cells * sizeof(double);
+    }
     int occ = 0;
     for (const auto& kv : h->occupancy) if (kv.first == plan.fn) occ = kv.second;
-    if (occ == 0) {
-        CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, 0));
+    if (occ == 0) {   // with the largest shared-memory footprint this kernel can be launched with
+        const size_t worst = diag ? static_cast<size_t>(plan.threads / 32) * kInlineItems * nq * sizeof(double) : 0;
+        CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, plan.fn, plan.threads, worst));
         if (occ < 1) occ = 1;
         h->occupancy.emplace_back(plan.fn, occ);
-    }
-    // per-warp diagnostic accumulators: [warps][items][5] doubles of dynamic shared memory
-    const size_t smem = diag ? static_cast<size_t>(plan.threads / 32) * n_items * kDiagQuantities * sizeof(double) : 0;
-    if (smem > 48 * 1024) {
-        size_t have = 0;
-        for (const auto& kv : h->smem_optin) if (kv.first == plan.fn) have = kv.second;
-        if (have < smem) {
-            CUDA_TRY(h, cudaFuncSetAttribute(plan.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-            h->smem_optin.emplace_back(plan.fn, smem);
-        }
     }
     int bps = h->blocks_per_sm > 0 ? h->blocks_per_sm : plan.blocks_per_sm;
     if (bps > occ) bps = occ;                      // persistent grid: never more than fit at once
@@ -118,19 +149,29 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
     if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;
     if (grid < 1) grid = 1;
 
+    {   // how many blocks work on any one item (the last block sums exactly their partials)
+        const long long n_tiles = (n_units + plan.tile_units - 1) / plan.tile_units;
+        long long per = grid;
+        if (a.tile_major) {
+            long long x = a.n_work, y = grid;
+            while (y) { const long long t = x % y; x = y; y = t; }   // x = gcd(n_work, grid)
+            per = grid / x;
+        }
+        a.touch_count = static_cast<int>(n_tiles < per ? n_tiles : per);
+    }
     void* params[] = {&a};
     CUDA_TRY(h, cudaLaunchKernel(plan.fn, dim3(static_cast<unsigned>(grid)), dim3(plan.threads), params, smem, h->stream));
     h->launches++;
     return HADPSGD_OK;
 }
 
-// All items of one mode over [elem_begin, elem_end); more than kMaxWork items (S > 480 unmixed
-// super-learners) take several launches.
+// All items of one mode over [elem_begin, elem_end); more than kInlineItems items (S > 64 paired or
+// S > 32 unmixed super-learners) take several launches.
 int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, bool shared_slots, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     if (elem_end <= elem_begin) return HADPSGD_OK;
-    for (size_t first = 0; first < items.size(); first += kMaxWork) {
-        const int n = static_cast<int>(items.size() - first < static_cast<size_t>(kMaxWork) ? items.size() - first : kMaxWork);
+    for (size_t first = 0; first < items.size(); first += kInlineItems) {
+        const int n = static_cast<int>(items.size() - first < static_cast<size_t>(kInlineItems) ? items.size() - first : kInlineItems);
         int rc = launch_chunk(h, items.data() + first, n, mode, shared_slots, lr, mu, elem_begin, elem_end, accumulate);
         if (rc != HADPSGD_OK) return rc;
     }
@@ -138,14 +179,13 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, b
 }
 
 // The launches of one step over the element range [elem_begin, elem_end).
-struct StepPlan { std::vector<WorkItem> pairs, singles; bool shared = false; };
-
 int step_range(hadpsgd_ctx* h, const StepPlan& sp, float lr, float mu, int64_t elem_begin, int64_t elem_end,
                bool accumulate) {
     const int pair_mode = (h->flags & HADPSGD_EQ7_LITERAL) ? kPairEq7 : kPair;
     int rc = launch_items(h, sp.pairs, pair_mode, sp.shared, lr, mu, elem_begin, elem_end, accumulate);
     if (rc != HADPSGD_OK) return rc;
-    // unmixed super-learners (S == 1, NO_MIX, or partner[s] == s in a custom matching)
+    // unmixed super-learners (S == 1, NO_MIX, or partner[s] == s in a custom matching), and in peer mode
+    // the members that publish u for a partner in another arena
     return launch_items(h, sp.singles, kSingle, false, lr, mu, elem_begin, elem_end, accumulate);
 }
 
@@ -165,18 +205,58 @@ int copy_slots(hadpsgd_ctx* h, const std::vector<SlotCopy>& copies) {
     return HADPSGD_OK;
 }
 
-// Matching -> work items with weight slots (updates h->w_slot) and enqueues any un-sharing copies.
-int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp) {
+// (Re)builds the device table of stage-buffer pointers: entry e * S_global + s_global.
+int upload_peer_table(hadpsgd_ctx* h) {
+    if (!h->peer_table_dirty) return HADPSGD_OK;
+    for (int r = 0; r < h->world; ++r)
+        if (!h->stage_of_rank[r]) { h->err = "rank " + std::to_string(r) + " is not attached (hadpsgd_peer_attach)"; return HADPSGD_INVALID_ARG; }
+    std::vector<const float*> tab(static_cast<size_t>(2) * h->S_global);
+    for (int r = 0; r < h->world; ++r) {
+        const int n = h->rank_begin[r + 1] - h->rank_begin[r];
+        for (int e = 0; e < 2; ++e)
+            for (int s = 0; s < n; ++s)
+                tab[static_cast<size_t>(e) * h->S_global + h->rank_begin[r] + s] =
+                    h->stage_of_rank[r] + (static_cast<size_t>(e) * n + s) * h->L.P_padded;
+    }
+    if (!h->d_peer) CUDA_TRY(h, cudaMalloc(reinterpret_cast<void**>(&h->d_peer), tab.size() * sizeof(float*)));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));   // no launch may still read the old table
+    CUDA_TRY(h, cudaMemcpy(h->d_peer, tab.data(), tab.size() * sizeof(float*), cudaMemcpyHostToDevice));
+    h->peer_table_dirty = false;
+    return HADPSGD_OK;
+}
+
+// Matching -> work items with weight buffers.  Nothing of the handle's state is committed here: the
+// caller commits `new_slot` / `new_pending` once every launch of the step has been enqueued.
+int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp, std::vector<int32_t>* new_slot,
+                     std::vector<int32_t>* new_pending) {
+    if (is_peer(h)) {
+        int rc = upload_peer_table(h);
+        if (rc != HADPSGD_OK) return rc;
+        *new_pending = h->pending;
+        rc = plan_peer_step(h->world, h->rank, h->rank_begin.data(), partner, h->epoch, new_pending, &sp->pairs, &sp->singles);
+        if (rc != HADPSGD_OK) { h->err = "peer plan failed: partner[] is not a matching of the S_global members"; return rc; }
+        sp->shared = false;
+        return HADPSGD_OK;
+    }
     const bool share = h->flags & HADPSGD_SHARE_PAIR_WEIGHTS;
     std::vector<SlotCopy> copies;
-    plan_step(h->L.S, partner, share, &h->w_slot, &sp->pairs, &sp->singles, &copies);
+    *new_slot = h->w_slot;
+    plan_step(h->L.S, partner, share, new_slot, &sp->pairs, &sp->singles, &copies);
     sp->shared = share;
-    h->last_n_pairs = static_cast<int>(sp->pairs.size());
     return copy_slots(h, copies);
 }
 
+void commit_plan(hadpsgd_ctx* h, const StepPlan& sp, const std::vector<int32_t>& new_slot,
+                 const std::vector<int32_t>& new_pending, uint64_t step_k) {
+    h->last_step_k = step_k;
+    h->last_n_pairs = static_cast<int>(sp.pairs.size());
+    if (is_peer(h)) { h->pending = new_pending; h->epoch++; }
+    else h->w_slot = new_slot;
+}
+
 int build_partner(hadpsgd_ctx* h, uint64_t step_k, const int32_t* custom, std::vector<int32_t>* partner) {
-    const int S = h->L.S;
+    const int S = is_peer(h) ? h->S_global : h->L.S;
+    if (is_peer(h) && !h->peer_init) { h->err = "HADPSGD_PEER handle: call hadpsgd_peer_init first"; return HADPSGD_INVALID_ARG; }
     partner->resize(S);
     if (custom) {
         if (validate_matching(S, custom) != HADPSGD_OK) { h->err = "partner[] is not a matching"; return HADPSGD_INVALID_ARG; }
@@ -231,9 +311,17 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
                          "not with NO_MIX or EQ7_LITERAL";
         return HADPSGD_INVALID_ARG;
     }
+    if (flags & HADPSGD_PEER) {
+        if (flags & (HADPSGD_SHARE_PAIR_WEIGHTS | HADPSGD_EQ7_LITERAL)) {
+            g_create_error = "HADPSGD_PEER cannot be combined with SHARE_PAIR_WEIGHTS or EQ7_LITERAL";
+            return HADPSGD_INVALID_ARG;
+        }
+        if (!dt.peer_stage) { g_create_error = "HADPSGD_PEER needs dtypes.peer_stage = 1 (the stage buffers)"; return HADPSGD_INVALID_ARG; }
+    }
     hadpsgd_ctx* h = new hadpsgd_ctx();
     h->w_slot.resize(S);
     for (int s = 0; s < S; ++s) h->w_slot[s] = s;
+    h->pending.assign(S, -1);
     h->L = L; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount;
     h->stream = opts ? static_cast<cudaStream_t>(opts->stream) : nullptr;
     if (opts && opts->arena) {
@@ -255,9 +343,10 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
         delete h; return HADPSGD_CUDA;
     }
     char* aux = h->arena + L.aux_off;
+    const int items = S < kMaxItemsPerLaunch ? S : kMaxItemsPerLaunch;
     h->d_partials = reinterpret_cast<double*>(aux);
-    h->d_diag = h->d_partials + static_cast<size_t>(S) * kDiagQuantities * kMaxGridBlocks;
-    h->d_ticket = reinterpret_cast<unsigned int*>(h->d_diag + 3 * S);
+    h->d_diag = h->d_partials + static_cast<size_t>(items) * kMaxDiagQuantities * kMaxGridBlocks;
+    h->d_ticket = reinterpret_cast<unsigned int*>(h->d_diag + kDiagArrays * S);
     *out = h;
     return HADPSGD_OK;
 }
@@ -268,6 +357,8 @@ extern "C" int hadpsgd_destroy(hadpsgd_handle h) {
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t ev : h->chunk_events) cudaEventDestroy(ev);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    if (h->d_peer) cudaFree(h->d_peer);
+    for (void* p : h->ipc_mapped) cudaIpcCloseMemHandle(p);
     if (h->owns_arena) cudaFree(h->arena);
     delete h;
     return HADPSGD_OK;
@@ -281,30 +372,26 @@ extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum,
                                      const int32_t* partner) {
     if (!h) return HADPSGD_INVALID_ARG;
     DeviceGuard guard(h->device);
-    std::vector<int32_t> pt;
-    int rc = build_partner(h, step_k, partner, &pt);
+    int rc = build_partner(h, step_k, partner, &h->partner);
     if (rc != HADPSGD_OK) return rc;
-    h->last_step_k = step_k;
-    StepPlan sp;
-    rc = plan_and_prepare(h, pt.data(), &sp);
+    std::vector<int32_t> new_slot, new_pending;
+    rc = plan_and_prepare(h, h->partner.data(), &h->plan, &new_slot, &new_pending);
     if (rc != HADPSGD_OK) return rc;
-    return step_range(h, sp, lr, momentum, 0, h->L.P_padded, false);
+    rc = step_range(h, h->plan, lr, momentum, 0, h->L.P_padded, false);
+    if (rc != HADPSGD_OK) return rc;
+    commit_plan(h, h->plan, new_slot, new_pending, step_k);   // only now: every launch is enqueued
+    return HADPSGD_OK;
 }
 
 extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads, float lr,
                                  float momentum, uint64_t step_k, hadpsgd_diag* diag_out) {
     if (!h || !host_grads) return HADPSGD_INVALID_ARG;
+    if (is_peer(h)) { h->err = "hadpsgd_step_host is not available on a HADPSGD_PEER handle"; return HADPSGD_INVALID_ARG; }
     DeviceGuard guard(h->device);
-    std::vector<int32_t> pt;
-    int rc = build_partner(h, step_k, nullptr, &pt);
+    int rc = build_partner(h, step_k, nullptr, &h->partner);
     if (rc != HADPSGD_OK) return rc;
-    h->last_step_k = step_k;
     const int n_buf = h->L.S * h->L.G;
     for (int b = 0; b < n_buf; ++b) if (!host_grads[b]) { h->err = "host_grads[] has a NULL entry"; return HADPSGD_INVALID_ARG; }
-
-    StepPlan sp;                      // one slot plan for the whole step, shared by all chunks
-    rc = plan_and_prepare(h, pt.data(), &sp);
-    if (rc != HADPSGD_OK) return rc;
 
     // Chunk the element range so the H2D copy of chunk c+1 overlaps the kernel on chunk c.
     const int64_t P = h->L.P_padded;
@@ -317,21 +404,43 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
         CUDA_TRY(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         h->chunk_events.push_back(ev);
     }
+
+    std::vector<int32_t> new_slot, new_pending;    // one slot plan for the whole step, shared by all chunks
+    rc = plan_and_prepare(h, h->partner.data(), &h->plan, &new_slot, &new_pending);
+    if (rc != HADPSGD_OK) return rc;
+
+    // On an error after this point copies from the caller's buffers may still be in flight and part of
+    // the step has run: drain both streams before reporting it, so the caller may free its buffers.
+    auto fail = [&](int code) {
+        cudaStreamSynchronize(h->copy_stream);
+        cudaStreamSynchronize(h->stream);
+        return code;
+    };
+#define CUDA_TRY_DRAIN(call)                                                                \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            h->err = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+            return fail(HADPSGD_CUDA);                                                      \
+        }                                                                                   \
+    } while (0)
     // the copy stream must not overwrite gradients an earlier step on h->stream still reads
-    CUDA_TRY(h, cudaEventRecord(h->chunk_events[n_chunks], h->stream));
-    CUDA_TRY(h, cudaStreamWaitEvent(h->copy_stream, h->chunk_events[n_chunks], 0));
+    CUDA_TRY_DRAIN(cudaEventRecord(h->chunk_events[n_chunks], h->stream));
+    CUDA_TRY_DRAIN(cudaStreamWaitEvent(h->copy_stream, h->chunk_events[n_chunks], 0));
     char* gdev = h->arena + h->L.g_off;
     for (int c = 0; c < n_chunks; ++c) {
         const int64_t e0 = c * chunk, e1 = (e0 + chunk < P) ? e0 + chunk : P;
         for (int b = 0; b < n_buf; ++b)
-            CUDA_TRY(h, cudaMemcpyAsync(gdev + static_cast<size_t>(b) * h->L.g_stride_bytes() + e0 * eb,
-                                        static_cast<const char*>(host_grads[b]) + e0 * eb,
-                                        static_cast<size_t>(e1 - e0) * eb, cudaMemcpyHostToDevice, h->copy_stream));
-        CUDA_TRY(h, cudaEventRecord(h->chunk_events[c], h->copy_stream));
-        CUDA_TRY(h, cudaStreamWaitEvent(h->stream, h->chunk_events[c], 0));
-        rc = step_range(h, sp, lr, momentum, e0, e1, c > 0);
-        if (rc != HADPSGD_OK) return rc;
+            CUDA_TRY_DRAIN(cudaMemcpyAsync(gdev + static_cast<size_t>(b) * h->L.g_stride_bytes() + e0 * eb,
+                                           static_cast<const char*>(host_grads[b]) + e0 * eb,
+                                           static_cast<size_t>(e1 - e0) * eb, cudaMemcpyHostToDevice, h->copy_stream));
+        CUDA_TRY_DRAIN(cudaEventRecord(h->chunk_events[c], h->copy_stream));
+        CUDA_TRY_DRAIN(cudaStreamWaitEvent(h->stream, h->chunk_events[c], 0));
+        rc = step_range(h, h->plan, lr, momentum, e0, e1, c > 0);
+        if (rc != HADPSGD_OK) return fail(rc);
     }
+#undef CUDA_TRY_DRAIN
+    commit_plan(h, h->plan, new_slot, new_pending, step_k);
     if (diag_out) return hadpsgd_diagnostics(h, diag_out);
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     return HADPSGD_OK;
@@ -339,6 +448,10 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
 
 extern "C" int hadpsgd_weights(hadpsgd_handle h, int s, float** dev_ptr) {
     if (!h || !dev_ptr || s < 0 || s >= h->L.S) return HADPSGD_INVALID_ARG;
+    if (is_peer(h) && h->pending[s] >= 0) {
+        h->err = "the mix of this super-learner with its partner in another arena is pending: call hadpsgd_peer_flush";
+        return HADPSGD_INVALID_ARG;
+    }
     *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.w_off + static_cast<size_t>(h->w_slot[s]) * h->L.w_stride_bytes());
     return HADPSGD_OK;
 }
@@ -375,31 +488,33 @@ extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
     if (h->flags & HADPSGD_NO_DIAG) { h->err = "handle was created with HADPSGD_NO_DIAG"; return HADPSGD_INVALID_ARG; }
     DeviceGuard guard(h->device);
     const int S = h->L.S;
-    std::vector<double> tmp(3 * S);
-    CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * 3 * S, cudaMemcpyDeviceToHost, h->stream));
+    std::vector<double> tmp(kDiagArrays * S);
+    CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * kDiagArrays * S, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     host_out->S = S; host_out->n_pairs = h->last_n_pairs; host_out->step_k = h->last_step_k;
     std::memcpy(host_out->gsq, tmp.data(), sizeof(double) * S);
     std::memcpy(host_out->wsq, tmp.data() + S, sizeof(double) * S);
     std::memcpy(host_out->gap, tmp.data() + 2 * S, sizeof(double) * S);
+    std::memcpy(host_out->pend_wsq, tmp.data() + 3 * S, sizeof(double) * S);
+    std::memcpy(host_out->pend_gap, tmp.data() + 4 * S, sizeof(double) * S);
+    for (int s = 0; s < S; ++s) host_out->pending[s] = (is_peer(h) && h->pending[s] >= 0) ? 1 : 0;
     return HADPSGD_OK;
-}
-
-namespace hadpsgd {
-int launch_consensus(const float* w, long long P_padded, int S, const int32_t* w_slot, int num_sms,
-                     double* block_out, cudaStream_t stream, cudaError_t* err);   // consensus.cu
 }
 
 extern "C" int hadpsgd_unshare(hadpsgd_handle h) {
     if (!h) return HADPSGD_INVALID_ARG;
     DeviceGuard guard(h->device);
     std::vector<SlotCopy> copies;
-    plan_unshare(h->L.S, &h->w_slot, &copies);
-    return copy_slots(h, copies);
+    std::vector<int32_t> slot = h->w_slot;
+    plan_unshare(h->L.S, &slot, &copies);
+    int rc = copy_slots(h, copies);
+    if (rc == HADPSGD_OK) h->w_slot = slot;
+    return rc;
 }
 
 extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
     if (!h || !D_out) return HADPSGD_INVALID_ARG;
+    if (is_peer(h)) { h->err = "hadpsgd_consensus needs all S_global weight columns in one arena: not on a HADPSGD_PEER handle"; return HADPSGD_INVALID_ARG; }
     DeviceGuard guard(h->device);
     // the partials scratch is free between steps: everything is ordered on h->stream
     cudaError_t e = cudaSuccess;
@@ -413,6 +528,108 @@ extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
     double D = 0.;
     for (int b = 0; b < grid; ++b) D += part[b];   // fixed order: run-to-run deterministic
     *D_out = D;
+    return HADPSGD_OK;
+}
+
+// ---- super-learner partition (row f4) ----------------------------------------------------
+
+extern "C" int hadpsgd_peer_init(hadpsgd_handle h, int rank, int world, const int32_t* rank_begin) {
+    if (!h || !rank_begin || world < 1 || rank < 0 || rank >= world) return HADPSGD_INVALID_ARG;
+    if (!is_peer(h)) { h->err = "handle was created without HADPSGD_PEER"; return HADPSGD_INVALID_ARG; }
+    if (h->epoch != 0) { h->err = "hadpsgd_peer_init after the first step"; return HADPSGD_INVALID_ARG; }
+    if (rank_begin[0] != 0) { h->err = "rank_begin[0] must be 0"; return HADPSGD_INVALID_ARG; }
+    for (int r = 0; r < world; ++r)
+        if (rank_begin[r + 1] <= rank_begin[r]) { h->err = "rank_begin must be increasing"; return HADPSGD_INVALID_ARG; }
+    if (rank_begin[world] > HADPSGD_MAX_S) { h->err = "S_global exceeds HADPSGD_MAX_S"; return HADPSGD_INVALID_ARG; }
+    if (rank_begin[rank + 1] - rank_begin[rank] != h->L.S) {
+        h->err = "this handle holds S = " + std::to_string(h->L.S) + " super-learners but rank_begin gives it " +
+                 std::to_string(rank_begin[rank + 1] - rank_begin[rank]);
+        return HADPSGD_INVALID_ARG;
+    }
+    h->rank = rank; h->world = world; h->S_global = rank_begin[world];
+    h->rank_begin.assign(rank_begin, rank_begin + world + 1);
+    h->stage_of_rank.assign(world, nullptr);
+    h->stage_of_rank[rank] = reinterpret_cast<const float*>(h->arena + h->L.stage_off);
+    h->peer_table_dirty = true;
+    h->peer_init = true;
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_peer_stage(hadpsgd_handle h, float** dev_ptr) {
+    if (!h || !dev_ptr) return HADPSGD_INVALID_ARG;
+    if (!is_peer(h)) { h->err = "handle was created without HADPSGD_PEER"; return HADPSGD_INVALID_ARG; }
+    *dev_ptr = reinterpret_cast<float*>(h->arena + h->L.stage_off);
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_peer_attach(hadpsgd_handle h, int r, const float* stage_region) {
+    if (!h || !stage_region) return HADPSGD_INVALID_ARG;
+    if (!is_peer(h) || !h->peer_init) { h->err = "call hadpsgd_peer_init first"; return HADPSGD_INVALID_ARG; }
+    if (r < 0 || r >= h->world || r == h->rank) { h->err = "rank out of range (or the handle's own rank)"; return HADPSGD_INVALID_ARG; }
+    h->stage_of_rank[r] = stage_region;
+    h->peer_table_dirty = true;
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_peer_ipc_export(hadpsgd_handle h, void* ipc_handle_out, uint64_t* stage_offset_out) {
+    if (!h || !ipc_handle_out || !stage_offset_out) return HADPSGD_INVALID_ARG;
+    if (!is_peer(h)) { h->err = "handle was created without HADPSGD_PEER"; return HADPSGD_INVALID_ARG; }
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "the ABI promises a 64-byte IPC handle");
+    DeviceGuard guard(h->device);
+    // The IPC handle names the whole ALLOCATION the arena lives in (a caller-supplied arena may be a
+    // slice of a larger one): find its base so that the importer can add the right offset.
+    void* base = nullptr;
+    {
+        using get_range_t = int (*)(unsigned long long*, size_t*, unsigned long long);
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        CUDA_TRY(h, cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qr));
+        if (!fn || qr != cudaDriverEntryPointSuccess) { h->err = "cuMemGetAddressRange is unavailable"; return HADPSGD_CUDA; }
+        unsigned long long b = 0; size_t sz = 0;
+        if (reinterpret_cast<get_range_t>(fn)(&b, &sz, reinterpret_cast<unsigned long long>(h->arena)) != 0) {
+            h->err = "cuMemGetAddressRange failed on the arena"; return HADPSGD_CUDA;
+        }
+        base = reinterpret_cast<void*>(b);
+    }
+    cudaIpcMemHandle_t ipc;
+    CUDA_TRY(h, cudaIpcGetMemHandle(&ipc, base));
+    std::memcpy(ipc_handle_out, &ipc, sizeof ipc);
+    *stage_offset_out = static_cast<uint64_t>(h->arena - static_cast<char*>(base)) + h->L.stage_off;
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_peer_ipc_attach(hadpsgd_handle h, int r, const void* ipc_handle, uint64_t stage_offset) {
+    if (!h || !ipc_handle) return HADPSGD_INVALID_ARG;
+    if (!is_peer(h) || !h->peer_init) { h->err = "call hadpsgd_peer_init first"; return HADPSGD_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    cudaIpcMemHandle_t ipc;
+    std::memcpy(&ipc, ipc_handle, sizeof ipc);
+    void* base = nullptr;
+    CUDA_TRY(h, cudaIpcOpenMemHandle(&base, ipc, cudaIpcMemLazyEnablePeerAccess));
+    h->ipc_mapped.push_back(base);
+    return hadpsgd_peer_attach(h, r, reinterpret_cast<const float*>(static_cast<char*>(base) + stage_offset));
+}
+
+extern "C" int hadpsgd_peer_flush(hadpsgd_handle h) {
+    if (!h) return HADPSGD_INVALID_ARG;
+    if (!is_peer(h) || !h->peer_init) { h->err = "call hadpsgd_peer_init first"; return HADPSGD_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    std::vector<int32_t> members;   // (local member, peer-table entry of the partner's stage buffer)
+    const int rd = static_cast<int>((h->epoch + 1) & 1);
+    for (int s = 0; s < h->L.S; ++s)
+        if (h->pending[s] >= 0) { members.push_back(s); members.push_back(rd * h->S_global + h->pending[s]); }
+    if (members.empty()) return HADPSGD_OK;
+    int rc = upload_peer_table(h);
+    if (rc != HADPSGD_OK) return rc;
+    cudaError_t e = cudaSuccess;
+    const float* a_stage = reinterpret_cast<const float*>(h->arena + h->L.stage_off) + static_cast<size_t>(rd) * h->L.S * h->L.P_padded;
+    launch_peer_flush(reinterpret_cast<float*>(h->arena + h->L.w_off), a_stage, h->d_peer, members.data(),
+                      static_cast<int>(members.size() / 2), h->L.P_padded, h->L.S, h->num_sms,
+                      (h->flags & HADPSGD_NO_DIAG) ? nullptr : h->d_partials, h->d_diag,
+                      (h->flags & HADPSGD_DETERMINISTIC) != 0, h->stream, &e);
+    CUDA_TRY(h, e);
+    h->launches++;
+    h->pending.assign(h->L.S, -1);
     return HADPSGD_OK;
 }
 

@@ -2,7 +2,7 @@
 #include "step_dispatch.cuh"
 
 namespace hadpsgd {
-LaunchPlan plan_f32(int G, bool exact, bool diag, int mode, bool shared) {
-    return pick_G<false, false>(G, exact, diag, mode, shared);
+LaunchPlan plan_f32(int G, bool exact, bool diag, int mode, int wmode) {
+    return pick_G<false, false>(G, exact, diag, mode, wmode);
 }
 }  // namespace hadpsgd

@@ -14,10 +14,19 @@
 // each byte is touched exactly once, so the design goal is only "the right amount of coalesced
 // 32 B requests in flight per SM" (~100 KB) and full-sector writes.
 //
+// Weight addressing (WMODE): every work item names, per member, the weight buffer it READS (a),
+// the buffer it WRITES (o) and -- in peer mode -- a second buffer b whose average with a IS the
+// member's weight: w = 1/2 (a + b).  That is how a pair whose members live in two arenas (two
+// GPUs; Fig. 3: one super-learner per node) is mixed without any kernel waiting
+// on another: at step k each side writes its u into a stage buffer instead of averaging, and
+// the launch of step k+1 forms 1/2 (u_own + u_partner) on the fly, reading the partner's stage
+// buffer through a peer pointer (NVLink) -- 4 B per parameter, inside this same fused pass.
+//
 // Diagnostics: per tile, per-thread sums -> warp shuffle tree -> the warp's own accumulator of
 // that work item in shared memory (no atomics, no block barrier per tile) -> at the end one block
 // partial per item in a fixed slot of global scratch -> the last block to finish (ticket) reduces
-// the partials in a fixed order.  Results are therefore run-to-run deterministic.
+// the partials in a fixed order.  Results are therefore run-to-run deterministic.  A launch of a
+// single block skips the scratch round trip and reduces straight from shared memory.
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -25,49 +34,52 @@
 
 namespace hadpsgd {
 
-constexpr int kMaxWork = 480;   // work items per launch: 480 x 8 B keeps StepArgs under 4 KB
-constexpr int kNQ = 5;  // gsq_a, gsq_b, wsq_a, wsq_b, gap
+constexpr int kInlineItems = 32;   // work items per launch (16 B each, inside the kernel parameter)
+constexpr int kNQ = 5;             // gsq_a, gsq_b, wsq_a, wsq_b, gap
+constexpr int kNQPeer = 9;         // ... + pend_wsq_a, pend_wsq_b, pend_gap_a, pend_gap_b (peer mode)
 
 enum Mode : int { kPair = 0, kSingle = 1, kPairEq7 = 2 };
+// kOwn: member s reads and writes weight buffer s.  kSlots: read buffer a, write buffer o (pair
+// members may share one buffer: HADPSGD_SHARE_PAIR_WEIGHTS).  kPeer: a, o and the pending-mix
+// partner buffer b (super-learner partition over several arenas / GPUs).
+enum WMode : int { kOwn = 0, kSlots = 1, kPeer = 2 };
+
+// Work item: super-learner indices s, p of the pair inside THIS handle (momentum and gradients
+// are always the member's own buffers); a_*: weight buffer index read; o_*: weight buffer index
+// written; b_*: 0, or 1 + index into StepArgs::peer of the buffer to average with a_* first.
+// Weight buffer index x addresses arena weights + x * P (main buffers 0..S-1, then -- peer mode
+// -- the 2S stage buffers).
+struct Item { unsigned short s, p, a_s, a_p, o_s, o_p, b_s, b_p; };
 
 struct StepArgs {
-    float* w;             // S buffers of P floats
+    float* w;             // weight buffers (main, then stage) of P floats each
     float* v;             // S buffers of P floats
     const void* g;        // S*G buffers of P grad elements
     void* wb;             // EMIT only: S buffers of P bf16, the working copy of the new weights
+    const float* const* peer;  // kPeer: device table of stage-buffer pointers (own and remote)
     long long P;          // padded elements per buffer
     long long unit_begin; // first vector unit of this launch
     long long unit_end;   // one past the last vector unit
+    double* partials;     // [gridDim.x][n_work * NQ]
+    double* diag;         // gsq[S] | wsq[S] | gap[S] | pend_wsq[S] | pend_gap[S]
+    unsigned int* ticket;
     int G;
     int n_work;
-    float lr, mu, invG;
-    int accumulate_diag;  // 0: diag = result ; 1: diag += result (chunked host path)
     int S;
-    double* partials;     // [n_work][kNQ][gridDim.x]
-    double* diag;         // gsq[S] | wsq[S] | gap[S]
-    unsigned int* ticket;
-    unsigned long long work[kMaxWork];   // six 10-bit fields per item, see pack_item()
+    int accumulate_diag;  // 0: diag = result ; 1: diag += result (chunked host path)
+    int tile_major;       // 0: item-major walk ; 1: tile-major (shared slots: L2 reuse)
+    int touch_count;      // blocks that work on any one item (host: from n_tiles, grid, walk order)
+    float lr, mu, invG;
+    Item items[kInlineItems];
 };
-
-// Work item = (s, p, ws, wp, wo_s, wo_p): super-learner indices of the pair (gradients and
-// momentum are always indexed by s / p), the weight slots w_s / w_p are READ from, and the slots
-// the new weights are WRITTEN to (wo_s == wo_p when the pair shares one copy).  S <= 512.
-__host__ __device__ inline unsigned long long pack_item(int s, int p, int ws, int wp, int wo_s, int wo_p) {
-    return static_cast<unsigned long long>(s) | static_cast<unsigned long long>(p) << 10 |
-           static_cast<unsigned long long>(ws) << 20 | static_cast<unsigned long long>(wp) << 30 |
-           static_cast<unsigned long long>(wo_s) << 40 | static_cast<unsigned long long>(wo_p) << 50;
-}
-struct Item { int s, p, ws, wp, wo_s, wo_p; };
-__device__ __forceinline__ Item unpack_item(unsigned long long w) {
-    return {static_cast<int>(w & 1023u), static_cast<int>((w >> 10) & 1023u), static_cast<int>((w >> 20) & 1023u),
-            static_cast<int>((w >> 30) & 1023u), static_cast<int>((w >> 40) & 1023u), static_cast<int>((w >> 50) & 1023u)};
-}
 
 // ---- memory access helpers -------------------------------------------------------------
 // Every byte is touched once per step, so all traffic is issued as 32-byte vector accesses
 // (ld/st.global.v8.b32, new on sm_100) carrying L2::evict_first: a warp covers 1 KB of each
 // stream per request, which measured ~6 % faster than 16-byte accesses on this path
-// because fewer, longer DRAM bursts are in flight per stream.
+// because fewer, longer DRAM bursts are in flight per stream.  (Selecting
+// the policy at run time -- evict_normal when one step's working set fits L2 -- measured no
+// faster at any L2-resident size and 0.4 % slower at full size, so the hint is a literal.)
 struct Raw8 { unsigned u[8]; };
 __device__ __forceinline__ Raw8 ld_stream32(const void* p) {
     Raw8 r;
@@ -142,9 +154,13 @@ __device__ __forceinline__ void store_state(float* base, long long off, const Ve
 }
 
 // EMIT: bf16 (round-to-nearest-even) copy of the new weights for mixed-precision learners
-// (SURVEY.md 8(f) row f2).  8 floats -> one 16 B store, 16 floats -> one 32 B store.
+// (SURVEY.md 8(f) row f2).  16 floats -> one 32 B store.  8 floats are only 16 B, so two
+// neighbouring lanes pair up: the even lane fetches its neighbour's four packed registers by
+// shuffle and stores 32 B for both (units come in even numbers -- P_padded and every sub-range are
+// multiples of 64 elements -- so an even lane's unit and the next are live or dead together).
+// Must be called by all 32 lanes of the warp; `live` predicates the store only.
 template <int UNIT>
-__device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<UNIT>& in) {
+__device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<UNIT>& in, bool live) {
     unsigned pk[UNIT / 2];
 #pragma unroll
     for (int q = 0; q < UNIT / 2; ++q) {
@@ -152,14 +168,18 @@ __device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<
         pk[q] = *reinterpret_cast<unsigned*>(&h);
     }
     __nv_bfloat16* dst = static_cast<__nv_bfloat16*>(base) + off;
+    Raw8 r;
     if constexpr (UNIT == 16) {
-        Raw8 r;
 #pragma unroll
         for (int q = 0; q < 8; ++q) r.u[q] = pk[q];
-        st_stream32(dst, r);
+        if (live) st_stream32(dst, r);
     } else {
-        // 16 B streaming store (an L2 evict-first cache-hint policy measured the same)
-        __stcs(reinterpret_cast<uint4*>(dst), make_uint4(pk[0], pk[1], pk[2], pk[3]));
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            r.u[q] = pk[q];
+            r.u[4 + q] = __shfl_down_sync(0xffffffffu, pk[q], 1);
+        }
+        if (live && (threadIdx.x & 1) == 0) st_stream32(dst, r);
     }
 }
 
@@ -226,6 +246,26 @@ template <int UNIT> __device__ __forceinline__ float sumsq(const Vec<UNIT>& a) {
     return s;
 }
 
+// Peer mode: the member's weight is the pending mix 1/2 (a + b) of its own stage buffer (already
+// in w) and its partner's (b, possibly in another GPU's memory); this IS phase 2 of the previous
+// step, 0.5f * (u_s + u_p).  Adds the two diagnostics that step still owes: sum m^2, sum (a-b)^2.
+template <bool EXACT, bool DIAG, int UNIT>
+__device__ __forceinline__ void resolve_pending(Vec<UNIT>& w, const Vec<UNIT>& b, double& d_wsq, double& d_gap) {
+    float sw = 0.f, sg = 0.f;
+#pragma unroll
+    for (int e = 0; e < UNIT; ++e) {
+        const float a = w.x[e];
+        const float m = mul_<EXACT>(0.5f, add_<EXACT>(a, b.x[e]));
+        if constexpr (DIAG) {
+            const float d = a - b.x[e];
+            sg = fmaf(d, d, sg);
+            sw = fmaf(m, m, sw);
+        }
+        w.x[e] = m;
+    }
+    if constexpr (DIAG) { d_wsq += static_cast<double>(sw); d_gap += static_cast<double>(sg); }
+}
+
 __device__ __forceinline__ double warp_sum(double x) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
@@ -244,19 +284,20 @@ __device__ __forceinline__ double warp_sum(double x) {
 // THREADS x U units; thread t owns units t, t+THREADS, ... of the tile, so each warp request
 // covers 1 KB contiguous of one stream.
 // ---------------------------------------------------------------------------------------
-// SHARED (kPair only): pair members share weight slots (HADPSGD_SHARE_PAIR_WEIGHTS): weights are
-// read from the item's read slots, the mixed weights are stored ONCE, and the walk is tile-major.
-template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, bool EMIT, bool SHARED, int U, int THREADS, int MINB>
+template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, bool EMIT, int WMODE, int U, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_constant__ StepArgs a) {
     constexpr int UNIT = BF16 ? 16 : 8;
     constexpr int GA = G > 0 ? G : 1;
     constexpr bool PAIRED = (MODE != kSingle);
-    // weights addressed through the item's slots: shared pairs, and every unmixed item (after an
-    // un-sharing copy the slot of an unmixed member need not be its own index)
-    constexpr bool SLOTS = SHARED || MODE == kSingle;
+    constexpr bool PEER = (WMODE == kPeer);
+    // weights addressed through the item's buffer indices: shared pairs, peer mode, and every
+    // unmixed item (after an un-sharing copy the buffer of an unmixed member need not be its own)
+    constexpr bool SLOTS = WMODE != kOwn || MODE == kSingle;
+    constexpr bool ONE_STORE = (WMODE == kSlots);   // pair members share ONE output buffer
     constexpr int NP = PAIRED ? U : 1;   // array extent of the partner's registers
     constexpr int WARPS = THREADS / 32;
-    extern __shared__ double s_acc[];    // DIAG: [WARPS][n_work][kNQ], each warp owns its rows
+    constexpr int NQ = PEER ? kNQPeer : kNQ;
+    extern __shared__ double s_acc[];    // DIAG: [WARPS][n_work][NQ], each warp owns its rows
     __shared__ unsigned int s_last;
 
     const int tid = threadIdx.x;
@@ -267,7 +308,7 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     constexpr long long TILE = static_cast<long long>(THREADS) * U;
 
     if constexpr (DIAG) {
-        for (int idx = tid; idx < WARPS * a.n_work * kNQ; idx += THREADS) s_acc[idx] = 0.;
+        for (int idx = tid; idx < WARPS * a.n_work * NQ; idx += THREADS) s_acc[idx] = 0.;
         __syncthreads();
     }
 
@@ -284,39 +325,52 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     // block barrier).  (Placing the hand-over after the next tile's loads, to hide its latency,
     // keeps all loads live across the shuffles and costs registers -- measured slower.)
     double d_gs = 0., d_gp = 0., d_ws = 0., d_wp = 0., d_gap = 0.;
+    double d_pws = 0., d_pwp = 0., d_pgs = 0., d_pgp = 0.;   // PEER: owed by the resolved pending mixes
     int cur = -1;
-    Item it = {0, 0, 0, 0, 0, 0};
+    unsigned touched = 0;    // bit j: this block worked on item j (n_work <= 32)
+    Item it = {0, 0, 0, 0, 0, 0, 0, 0};
     // element offsets of the current item's buffers, recomputed only when the item changes
     long long o_vs = 0, o_vp = 0, o_gs = 0, o_gp = 0;   // momentum / gradients: the member's own buffers
-    long long o_ws = 0, o_wp = 0, o_wo = 0;             // SHARED: weight read slots and the one write slot
+    long long o_ws = 0, o_wp = 0, o_wos = 0, o_wop = 0; // SLOTS: weight read buffers and write buffers
+    const float* pb_s = nullptr;                        // PEER: pending-mix partner buffers (or null)
+    const float* pb_p = nullptr;
     auto hand_over = [&](int item) {
         if constexpr (MODE == kPair) d_wp = d_ws;
-        double q[kNQ] = {d_gs, d_gp, d_ws, d_wp, d_gap};
+        double q[NQ];
+        q[0] = d_gs; q[1] = d_gp; q[2] = d_ws; q[3] = d_wp; q[4] = d_gap;
+        if constexpr (PEER) { q[5] = d_pws; q[6] = d_pwp; q[7] = d_pgs; q[8] = d_pgp; }
 #pragma unroll
-        for (int k = 0; k < kNQ; ++k) q[k] = warp_sum(q[k]);
+        for (int k = 0; k < NQ; ++k) q[k] = warp_sum(q[k]);
         if ((tid & 31) == 0) {
-            double* row = s_acc + (static_cast<size_t>(tid >> 5) * a.n_work + item) * kNQ;
+            double* row = s_acc + (static_cast<size_t>(tid >> 5) * a.n_work + item) * NQ;
 #pragma unroll
-            for (int k = 0; k < kNQ; ++k) row[k] += q[k];
+            for (int k = 0; k < NQ; ++k) row[k] += q[k];
         }
         d_gs = d_gp = d_ws = d_wp = d_gap = 0.;
+        d_pws = d_pwp = d_pgs = d_pgp = 0.;
     };
     for (long long gt = blockIdx.x; gt < total_tiles; gt += gridDim.x) {
         int j;
         long long tile;
-        if constexpr (SHARED) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
+        if (WMODE == kSlots && a.tile_major) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
         else { j = static_cast<int>(gt / n_tiles); tile = gt - static_cast<long long>(j) * n_tiles; }
         const long long base = tile * TILE;
         if (j != cur) {                                  // block-uniform
             if constexpr (DIAG) { if (cur >= 0) hand_over(cur); }
             cur = j;
-            it = unpack_item(a.work[j]);
+            touched |= 1u << j;
+            it = a.items[j];
             o_vs = it.s * P; o_vp = it.p * P;
             o_gs = o_vs * a.G; o_gp = o_vp * a.G;               // learner 0 of each member
-            if constexpr (SLOTS) { o_ws = it.ws * P; o_wp = it.wp * P; o_wo = it.wo_s * P; }
+            if constexpr (SLOTS) { o_ws = it.a_s * P; o_wp = it.a_p * P; o_wos = it.o_s * P; o_wop = it.o_p * P; }
+            if constexpr (PEER) {
+                pb_s = it.b_s ? a.peer[it.b_s - 1] : nullptr;
+                pb_p = (PAIRED && it.b_p) ? a.peer[it.b_p - 1] : nullptr;
+            }
         }
         {
             Vec<UNIT> ws[U], vs[U], gbs[U], wp[NP], vp[NP], gbp[NP];
+            Vec<UNIT> bs[PEER ? U : 1], bp[PEER ? NP : 1];
             bool live[U];
             long long elem[U];
 #pragma unroll
@@ -340,6 +394,10 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                             load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
                             load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
+                        if constexpr (PEER) {
+                            if (pb_s) load_state<UNIT>(pb_s, elem[q], bs[q]);
+                            if constexpr (PAIRED) { if (pb_p) load_state<UNIT>(pb_p, elem[q], bp[q]); }
+                        }
                     }
                 }
 #pragma unroll
@@ -359,6 +417,10 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                             load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
                             load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
+                        if constexpr (PEER) {
+                            if (pb_s) load_state<UNIT>(pb_s, elem[q], bs[q]);
+                            if constexpr (PAIRED) { if (pb_p) load_state<UNIT>(pb_p, elem[q], bp[q]); }
+                        }
                         sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, o_gs + elem[q], gbs[q]);
                         if constexpr (PAIRED) sum_grads_runtime<BF16, EXACT, UNIT>(gbytes, P, a.G, o_gp + elem[q], gbp[q]);
                     }
@@ -367,56 +429,64 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 
 #pragma unroll
             for (int q = 0; q < U; ++q) {
-                if (!live[q]) continue;
                 const long long os = o_vs + elem[q];
                 const long long op = o_vp + elem[q];
+                const long long wos = SLOTS ? o_wos + elem[q] : os;
+                const long long wop = SLOTS ? o_wop + elem[q] : op;
                 Vec<UNIT> us, up, outs, outp, dif;
-                apply_update<EXACT, UNIT>(gbs[q], invG, mu, lr, ws[q], vs[q], us);
-                if constexpr (PAIRED) apply_update<EXACT, UNIT>(gbp[q], invG, mu, lr, wp[q], vp[q], up);
+                if (live[q]) {
+                    if constexpr (PEER) {   // finish the previous step's mix across arenas first
+                        if (pb_s) resolve_pending<EXACT, DIAG, UNIT>(ws[q], bs[q], d_pws, d_pgs);
+                        if constexpr (PAIRED) { if (pb_p) resolve_pending<EXACT, DIAG, UNIT>(wp[q], bp[q], d_pwp, d_pgp); }
+                    }
+                    apply_update<EXACT, UNIT>(gbs[q], invG, mu, lr, ws[q], vs[q], us);
+                    if constexpr (PAIRED) apply_update<EXACT, UNIT>(gbp[q], invG, mu, lr, wp[q], vp[q], up);
 
-                // a4: pairwise average.  Default (R3): both members get 1/2 (u_s + u_p).
-                // kPairEq7: eq. (7) as printed, w'_s = 1/2 (w_s + w_p) - lr v'_s.
-                if constexpr (MODE == kPair) {
+                    // a4: pairwise average.  Default (R3): both members get 1/2 (u_s + u_p).
+                    // kPairEq7: eq. (7) as printed, w'_s = 1/2 (w_s + w_p) - lr v'_s.
+                    if constexpr (MODE == kPair) {
 #pragma unroll
-                    for (int e = 0; e < UNIT; ++e) {
-                        float m = mul_<EXACT>(0.5f, add_<EXACT>(us.x[e], up.x[e]));
-                        outs.x[e] = m;
-                        if constexpr (DIAG) dif.x[e] = us.x[e] - up.x[e];
-                    }
-                } else if constexpr (MODE == kPairEq7) {
+                        for (int e = 0; e < UNIT; ++e) {
+                            float m = mul_<EXACT>(0.5f, add_<EXACT>(us.x[e], up.x[e]));
+                            outs.x[e] = m;
+                            if constexpr (DIAG) dif.x[e] = us.x[e] - up.x[e];
+                        }
+                    } else if constexpr (MODE == kPairEq7) {
 #pragma unroll
-                    for (int e = 0; e < UNIT; ++e) {
-                        float m = mul_<EXACT>(0.5f, add_<EXACT>(ws[q].x[e], wp[q].x[e]));
-                        // recover lr v' the same way the oracle does (one fp32 multiply)
-                        float ts = mul_<EXACT>(lr, vs[q].x[e]), tp = mul_<EXACT>(lr, vp[q].x[e]);
-                        outs.x[e] = EXACT ? __fsub_rn(m, ts) : m - ts;
-                        outp.x[e] = EXACT ? __fsub_rn(m, tp) : m - tp;
-                        if constexpr (DIAG) dif.x[e] = ws[q].x[e] - wp[q].x[e];
+                        for (int e = 0; e < UNIT; ++e) {
+                            float m = mul_<EXACT>(0.5f, add_<EXACT>(ws[q].x[e], wp[q].x[e]));
+                            // recover lr v' the same way the oracle does (one fp32 multiply)
+                            float ts = mul_<EXACT>(lr, vs[q].x[e]), tp = mul_<EXACT>(lr, vp[q].x[e]);
+                            outs.x[e] = EXACT ? __fsub_rn(m, ts) : m - ts;
+                            outp.x[e] = EXACT ? __fsub_rn(m, tp) : m - tp;
+                            if constexpr (DIAG) dif.x[e] = ws[q].x[e] - wp[q].x[e];
+                        }
+                    } else {
+                        outs = us;
                     }
-                } else {
-                    outs = us;
-                }
 
-                const long long wos = SLOTS ? o_wo + elem[q] : os;
-                store_state<UNIT>(a.v, os, vs[q]);
-                store_state<UNIT>(a.w, wos, outs);
-                if constexpr (EMIT) store_bf16<UNIT>(a.wb, wos, outs);
-                if constexpr (PAIRED) {
-                    store_state<UNIT>(a.v, op, vp[q]);
-                    if constexpr (!SHARED) {       // pair members keep separate copies
-                        store_state<UNIT>(a.w, op, MODE == kPair ? outs : outp);
-                        if constexpr (EMIT) store_bf16<UNIT>(a.wb, op, MODE == kPair ? outs : outp);
-                    }
-                }
-
-                if constexpr (DIAG) {
-                    d_gs += static_cast<double>(sumsq<UNIT>(gbs[q]));
-                    d_ws += static_cast<double>(sumsq<UNIT>(outs));
+                    store_state<UNIT>(a.v, os, vs[q]);
+                    store_state<UNIT>(a.w, wos, outs);
                     if constexpr (PAIRED) {
-                        d_gp += static_cast<double>(sumsq<UNIT>(gbp[q]));
-                        d_gap += static_cast<double>(sumsq<UNIT>(dif));
-                        if constexpr (MODE == kPairEq7) d_wp += static_cast<double>(sumsq<UNIT>(outp));
+                        store_state<UNIT>(a.v, op, vp[q]);
+                        if constexpr (!ONE_STORE)       // pair members keep separate copies
+                            store_state<UNIT>(a.w, wop, MODE == kPair ? outs : outp);
                     }
+
+                    if constexpr (DIAG) {
+                        d_gs += static_cast<double>(sumsq<UNIT>(gbs[q]));
+                        d_ws += static_cast<double>(sumsq<UNIT>(outs));
+                        if constexpr (PAIRED) {
+                            d_gp += static_cast<double>(sumsq<UNIT>(gbp[q]));
+                            d_gap += static_cast<double>(sumsq<UNIT>(dif));
+                            if constexpr (MODE == kPairEq7) d_wp += static_cast<double>(sumsq<UNIT>(outp));
+                        }
+                    }
+                }
+                if constexpr (EMIT) {     // outside `live`: the lanes of a warp shuffle together
+                    store_bf16<UNIT>(a.wb, wos, outs, live[q]);
+                    if constexpr (PAIRED && !ONE_STORE)
+                        store_bf16<UNIT>(a.wb, wop, MODE == kPair ? outs : outp, live[q]);
                 }
             }
         }
@@ -425,17 +495,51 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 
     if constexpr (DIAG) {
         if (cur >= 0) hand_over(cur);
-        // block partial of every item (zero for items this block never touched) -> partials[j][q][block]
         __syncthreads();
-        for (int idx = tid; idx < a.n_work * kNQ; idx += THREADS) {
-            double tot = 0.;
-            for (int wi = 0; wi < WARPS; ++wi) tot += s_acc[static_cast<size_t>(wi) * a.n_work * kNQ + idx];  // fixed order
-            a.partials[static_cast<size_t>(idx) * gridDim.x + blockIdx.x] = tot;
+        const int R = a.n_work * NQ;     // rows: (item, quantity)
+        // row -> its place in the result.  k: 0 gsq_s, 1 gsq_p, 2 wsq_s, 3 wsq_p, 4 gap (reported for
+        // both members), 5-8 (peer) the wsq / gap a resolved pending mix owes to the step before
+        auto publish = [&](int row, double sum) {
+            const int j = row / NQ, k = row - j * NQ;
+            const Item w = a.items[j];
+            const int s = w.s, p = w.p, S = a.S;
+            double* gsq = a.diag; double* wsq = a.diag + S; double* gap = a.diag + 2 * S;
+            auto put = [&](double* dst, double val) { *dst = a.accumulate_diag ? *dst + val : val; };
+            if (k == 0) put(gsq + s, sum);
+            if (k == 2) put(wsq + s, sum);
+            if (PAIRED) {
+                if (k == 1) put(gsq + p, sum);
+                if (k == 3) put(wsq + p, sum);
+                if (k == 4) { put(gap + s, sum); put(gap + p, sum); }
+            } else if (k == 4) {
+                put(gap + s, 0.0);
+            }
+            if constexpr (PEER) {
+                double* pws = a.diag + 3 * S; double* pgp = a.diag + 4 * S;
+                if (k == 5) put(pws + s, sum);
+                if (k == 7) put(pgp + s, sum);
+                if (PAIRED) {
+                    if (k == 6) put(pws + p, sum);
+                    if (k == 8) put(pgp + p, sum);
+                }
+            }
+        };
+        if (gridDim.x == 1) {            // the only block: its warp rows ARE the result
+            for (int row = tid; row < R; row += THREADS) {
+                double tot = 0.;
+                for (int wi = 0; wi < WARPS; ++wi) tot += s_acc[static_cast<size_t>(wi) * R + row];   // fixed order
+                publish(row, tot);
+            }
+            return;
         }
-    }
-
-    if constexpr (DIAG) {
-        // last block to arrive reduces all block partials in a fixed order.  Order matters: every
+        // block partial of the rows of every item this block worked on -> partials[block][row]
+        for (int row = tid; row < R; row += THREADS) {
+            if (!((touched >> (row / NQ)) & 1u)) continue;
+            double tot = 0.;
+            for (int wi = 0; wi < WARPS; ++wi) tot += s_acc[static_cast<size_t>(wi) * R + row];       // fixed order
+            a.partials[static_cast<size_t>(blockIdx.x) * R + row] = tot;
+        }
+        // The last block to arrive reduces all block partials in a fixed order.  Order matters: every
         // thread's partial stores, then its fence, then a block barrier, and only then the ticket --
         // otherwise warp 0 could publish the ticket before another warp's partials are out.
         __threadfence();
@@ -445,34 +549,43 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             s_last = (t == gridDim.x - 1) ? 1u : 0u;
         }
         __syncthreads();
-        if (s_last) {
-            __threadfence();
-            const int lane = tid & 31, wid = tid >> 5;
-            for (int item = wid; item < a.n_work * kNQ; item += THREADS / 32) {
-                const double* src = a.partials + static_cast<size_t>(item) * gridDim.x;
-                double sum = 0.;
-                for (unsigned b = lane; b < gridDim.x; b += 32) sum += __ldcg(src + b);
-                sum = warp_sum(sum);
-                if (lane == 0) {
-                    const int j = item / kNQ, k = item % kNQ;
-                    const Item it = unpack_item(a.work[j]);
-                    const int s = it.s, p = it.p;
-                    // k: 0 gsq_s, 1 gsq_p, 2 wsq_s, 3 wsq_p, 4 gap (reported for both members)
-                    double* gsq = a.diag; double* wsq = a.diag + a.S; double* gap = a.diag + 2 * a.S;
-                    auto put = [&](double* dst, double val) { *dst = a.accumulate_diag ? *dst + val : val; };
-                    if (k == 0) put(gsq + s, sum);
-                    if (k == 2) put(wsq + s, sum);
-                    if (PAIRED) {
-                        if (k == 1) put(gsq + p, sum);
-                        if (k == 3) put(wsq + p, sum);
-                        if (k == 4) { put(gap + s, sum); put(gap + p, sum); }
-                    } else if (k == 4) {
-                        put(gap + s, 0.0);
-                    }
-                }
+        if (!s_last) return;
+        __threadfence();
+        // Item j was worked on by exactly touch_count blocks: the i-th of them (in tile order) is block
+        // (j * n_tiles + i) mod grid in the item-major walk, (i * n_work + j) mod grid in the tile-major
+        // one.  Only their partials are read (for a small problem that is one block per tile instead of
+        // the whole grid), with every thread busy: thread (c, row) sums contributors c, c+C, c+2C, ... of
+        // its row (independent loads), then the C column sums of a row are added in order.  The result
+        // depends on the launch shape only: run-to-run deterministic.
+        const int C = (THREADS / R) > 0 ? (THREADS / R) : 1;
+        double* s_col = s_acc;           // reuse: C x R <= max(THREADS, R) doubles (the host sizes it)
+        const unsigned nb = gridDim.x;
+        const bool tmaj = (WMODE == kSlots) && a.tile_major;
+        // contributor i of item j is block (first + i * step) mod nb; walked incrementally (no division
+        // inside the loop)
+        const unsigned step1 = tmaj ? static_cast<unsigned>(a.n_work) % nb : 1u % nb;
+        const unsigned stepC = static_cast<unsigned>((static_cast<unsigned long long>(step1) * C) % nb);
+        for (int task = tid; task < R * C; task += THREADS) {
+            const int c = task / R, row = task - c * R;
+            const unsigned j = row / NQ;
+            const unsigned long long first = tmaj ? j : static_cast<unsigned long long>(j) * static_cast<unsigned long long>(n_tiles);
+            unsigned b = static_cast<unsigned>((first + static_cast<unsigned long long>(step1) * c) % nb);
+            double sum = 0.;
+#pragma unroll 4
+            for (int i = c; i < a.touch_count; i += C) {
+                sum += __ldcg(a.partials + static_cast<size_t>(b) * R + row);
+                b += stepC;
+                if (b >= nb) b -= nb;
             }
-            if (tid == 0) *a.ticket = 0u;  // re-arm for the next launch on this stream
+            s_col[task] = sum;
         }
+        __syncthreads();
+        for (int row = tid; row < R; row += THREADS) {
+            double sum = 0.;
+            for (int c = 0; c < C; ++c) sum += s_col[c * R + row];
+            publish(row, sum);
+        }
+        if (tid == 0) *a.ticket = 0u;  // re-arm for the next launch on this stream
     }
 }
 

@@ -61,7 +61,7 @@ def test_allocator_layout(H):
     assert lay["P_padded"] == P and lay["seg_offset"] == [0]
     assert lay["w_off"] == 0 and lay["v_off"] == 16 * P * 4 and lay["g_off"] == 32 * P * 4
     need = H.hadpsgd_required_bytes(16, 4, [P])
-    assert 16 * P * (4 * 4 + 8) <= need <= 16 * P * (4 * 4 + 8) + (4 << 20)
+    assert 16 * P * (4 * 4 + 8) <= need <= 16 * P * (4 * 4 + 8) + (16 << 20)      # + diagnostics scratch
     # ragged bf16 config 3: 40 segments, every natural length is a multiple of 64 -> no padding
     seg = [n for _, n in shapes.SWB2000_SEGMENTS]
     lay = H.hadpsgd_layout(8, 8, seg, H.BF16)

@@ -303,6 +303,231 @@ def test_share_pair_weights_graph_replay_from_steady_state(H, oracle_mod, torch_
     h.close()
 
 
+# ------------------------------------------------------------------------------- super-learner partition (f4)
+
+def _ring(S, k):
+    p = [0] * S
+    for i in range(S // 2):
+        a, b = (2 * i + k % 2) % S, (2 * i + 1 + k % 2) % S
+        p[a], p[b] = b, a
+    return p
+
+
+def run_peer_group(H, oracle_mod, rank_begin, G, seg_len, matchings, *, bf16=False, exact=True, seed=401,
+                   flush_at=(), no_diag=False):
+    """R = len(rank_begin)-1 HADPSGD_PEER handles on ONE GPU and one stream stand in for R ranks (a
+    same-device pointer is a valid peer pointer; one stream is the epoch barrier).  Every step is
+    compared with the oracle on all S_global super-learners: momentum and gsq at once; weights, wsq and
+    gap at once for members whose mix completed inside the step, and one step later (pend_wsq /
+    pend_gap, or after hadpsgd_peer_flush) for members whose partner lives in another arena."""
+    import torch
+    from fixtures import device, generator as gen
+    world, S = len(rank_begin) - 1, rank_begin[-1]
+    P = int(sum(seg_len))
+    flags = H.PEER | (H.DETERMINISTIC if exact else 0) | (H.NO_DIAG if no_diag else 0)
+    hs = [H.Hadpsgd(rank_begin[r + 1] - rank_begin[r], G, seg_len, H.BF16 if bf16 else H.F32, flags) for r in range(world)]
+    for r, h in enumerate(hs):
+        h.hadpsgd_peer_init(r, world, rank_begin)
+    for r, h in enumerate(hs):
+        for q, other in enumerate(hs):
+            if q != r:
+                h.hadpsgd_peer_attach(q, other.hadpsgd_peer_stage())
+    nat_off = np.concatenate([[0], np.cumsum(seg_len)])
+
+    def fill(buf, h, key, dist, scale):
+        for k, n in enumerate(seg_len):
+            off, _ = h.hadpsgd_segment(k)
+            device.fill(buf[off:off + n], key, dist, scale, elem_offset=int(nat_off[k]))
+
+    owner = lambda sg: next(r for r in range(world) if rank_begin[r] <= sg < rank_begin[r + 1])
+    for sg in range(S):
+        h = hs[owner(sg)]
+        fill(h.hadpsgd_weights(sg - rank_begin[owner(sg)]), h, gen.stream_key(seed, gen.STREAM_WEIGHT, 0, sg, 0), "normal", 0.05)
+    from fixtures import problem
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    nat = torch.from_numpy(hs[0].natural_index()).cuda()
+    prev = None                                       # (oracle diag, pending flags) of the step before
+    for k, partner in enumerate(matchings):
+        for sg in range(S):
+            h, sl = hs[owner(sg)], sg - rank_begin[owner(sg)]
+            for g in range(G):
+                fill(h.hadpsgd_grads(sl, g), h, gen.stream_key(seed, gen.STREAM_GRAD, k, sg, g), "normal", 1e-3)
+        for h in hs:                                  # same stream: launch order is the epoch barrier
+            if partner is None:
+                h.hadpsgd_step(LR, MU, k)
+            else:
+                h.hadpsgd_step_matching(LR, MU, k, partner)
+        og = problem.host_grads(seed, k, S, G, 0, P, bf16=bf16)
+        od = oracle_mod.step(og, ow, ov, LR, MU, k, diag=True, partner=partner if partner is not None else _ring(S, k))
+        pend_now = np.zeros(S, bool)
+        for r, h in enumerate(hs):
+            lo, hi = rank_begin[r], rank_begin[r + 1]
+            gv = np.stack([h.hadpsgd_momentum(s)[nat].cpu().numpy() for s in range(hi - lo)])
+            if exact:
+                assert np.array_equal(bits(gv), bits(ov[lo:hi])), (k, r)
+            else:
+                assert np.all(np.abs(gv - ov[lo:hi]) <= 1e-6 + 1e-5 * np.abs(ov[lo:hi]))
+            if no_diag:
+                continue
+            d = h.hadpsgd_diagnostics()
+            pend_now[lo:hi] = d["pending"] == 1
+            assert np.allclose(d["gsq"], od["gsq"][lo:hi], rtol=1e-4, atol=1e-30), (k, r)
+            done = ~pend_now[lo:hi]
+            assert np.allclose(d["wsq"][done], od["wsq"][lo:hi][done], rtol=1e-4, atol=1e-30), (k, r)
+            assert np.allclose(d["gap"][done], od["gap"][lo:hi][done], rtol=1e-4, atol=1e-30), (k, r)
+            assert np.array_equal(d["gap"][done] == 0, od["gap"][lo:hi][done] == 0)
+            if prev is not None:                      # what the step before still owed
+                was = prev[1][lo:hi]
+                assert np.allclose(d["pend_wsq"][was], prev[0]["wsq"][lo:hi][was], rtol=1e-4), (k, r)
+                assert np.allclose(d["pend_gap"][was], prev[0]["gap"][lo:hi][was], rtol=1e-4), (k, r)
+                assert not d["pend_wsq"][~was].any() and not d["pend_gap"][~was].any()
+        prev = (od, pend_now)
+        if k in flush_at:
+            for r, h in enumerate(hs):
+                h.hadpsgd_peer_flush()
+                if not no_diag:
+                    d = h.hadpsgd_diagnostics()
+                    lo, hi = rank_begin[r], rank_begin[r + 1]
+                    was = pend_now[lo:hi]
+                    assert np.allclose(d["pend_wsq"][was], od["wsq"][lo:hi][was], rtol=1e-4)
+                    assert np.allclose(d["pend_gap"][was], od["gap"][lo:hi][was], rtol=1e-4)
+                    assert not d["pending"].any()
+            prev = None
+            gw = np.concatenate([np.stack([h.hadpsgd_weights(s)[nat].cpu().numpy() for s in range(h.S)]) for h in hs])
+            assert_parity(gw, gw * 0, ow, ow * 0, exact)
+    for h in hs:
+        h.hadpsgd_peer_flush()
+    torch.cuda.synchronize()
+    gw = np.concatenate([np.stack([h.hadpsgd_weights(s)[nat].cpu().numpy() for s in range(h.S)]) for h in hs])
+    gv = np.concatenate([np.stack([h.hadpsgd_momentum(s)[nat].cpu().numpy() for s in range(h.S)]) for h in hs])
+    launches = [h.hadpsgd_launch_count() for h in hs]
+    if sum(seg_len) != hs[0].P_padded:                # padding of main and stage buffers stays zero
+        mask = torch.ones(hs[0].P_padded, dtype=torch.bool, device="cuda"); mask[nat] = False
+        for h in hs:
+            stage = h._view(h.hadpsgd_peer_stage(), 2 * h.S * h.P_padded, torch.float32).view(2 * h.S, h.P_padded)
+            assert not stage[:, mask].any()
+    for h in hs:
+        h.close()
+    assert_parity(gw, gv, ow, ov, exact)
+    return launches
+
+
+@pytest.mark.parametrize("rank_begin", [[0, 2, 4, 6, 8], [0, 1, 2, 3, 4], [0, 3, 5, 8], [0, 8], [0, 4, 8]])
+@pytest.mark.parametrize("exact", [True, False])
+def test_peer_partition_ring_multi_arena(H, oracle_mod, rank_begin, exact):
+    """Ring schedule over R arenas (2 super-learners per 'GPU' is the paper's 16x4 on 8 nodes in small):
+    on odd steps EVERY pair straddles two arenas.  Ragged table, 7 steps, a flush in the middle."""
+    run_peer_group(H, oracle_mod, rank_begin, 4, ODD_TABLE, [None] * 7, exact=exact, flush_at=(3,))
+
+
+def test_peer_partition_custom_matchings_odd_S(H, oracle_mod):
+    rank_begin = [0, 3, 4, 7]
+    matchings = [[3, 1, 5, 0, 4, 2, 6], [1, 0, 3, 2, 5, 4, 6], [6, 2, 1, 4, 3, 5, 0], [0, 1, 2, 3, 4, 5, 6],
+                 [4, 5, 6, 3, 0, 1, 2], [4, 5, 6, 3, 0, 1, 2], [1, 0, 2, 6, 5, 4, 3]]
+    run_peer_group(H, oracle_mod, rank_begin, 2, [50_003], matchings, flush_at=(2, 4))
+
+
+@pytest.mark.parametrize("G,bf16", [(8, True), (3, False), (8, False), (1, True)])
+def test_peer_partition_other_kernels(H, oracle_mod, G, bf16):
+    """bf16 gradients, G = 8 and the runtime-G kernel in peer mode; one launch per step per rank when a
+    rank's work is all pairs or all singles."""
+    launches = run_peer_group(H, oracle_mod, [0, 2, 4], G, [70_001], [None] * 4, bf16=bf16)
+    assert launches == [4 + 1, 4 + 1]                  # 4 steps + the final flush (S = 4: both members pending)
+    run_peer_group(H, oracle_mod, [0, 2, 4], G, [3_001], [None] * 3, bf16=bf16, no_diag=True)
+
+
+def test_peer_errors(H):
+    h = H.Hadpsgd(2, 2, [1000], H.F32, H.PEER)
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_step(LR, MU, 0)                       # not initialised
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_peer_init(0, 2, [0, 3, 4])            # S mismatch
+    h.hadpsgd_peer_init(0, 2, [0, 2, 4])
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_step(LR, MU, 1)                       # rank 1 not attached
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_peer_attach(0, h.hadpsgd_peer_stage())   # own rank
+    with pytest.raises(H.HadpsgdError):
+        h.hadpsgd_consensus()
+    h.close()
+    for bad in (H.SHARE_PAIR_WEIGHTS, H.EQ7_LITERAL):
+        with pytest.raises(H.HadpsgdError):
+            H.Hadpsgd(2, 2, [1000], H.F32, H.PEER | bad)
+    with pytest.raises(H.HadpsgdError):
+        H.Hadpsgd(2, 2, [1000], H.F32, H.PEER, working_dtype=H.BF16)
+    plain = H.Hadpsgd(2, 2, [1000])
+    with pytest.raises(H.HadpsgdError):
+        plain.hadpsgd_peer_init(0, 1, [0, 2])
+    plain.close()
+
+
+def _ipc_worker(rank, world, port, out_dir):
+    """One process per rank, BOTH ON GPU 0: stage regions are exchanged as CUDA IPC handles (gloo carries
+    the 64 bytes), the epoch barrier is synchronize + a gloo barrier.  No kernel waits on another."""
+    import os
+    import torch
+    import torch.distributed as dist
+    import paper_1907_05701_b200 as Hm
+    from fixtures import device, generator as gen
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        S, G, P, seed, steps = 8, 2, 200_003, 431, 5
+        rank_begin = [0, 4, 8]
+        lo = rank_begin[rank]
+        h = Hm.Hadpsgd(4, G, [P], Hm.F32, Hm.PEER | Hm.DETERMINISTIC, own_arena=(rank == 0))   # one of each arena kind
+        h.hadpsgd_peer_init(rank, world, rank_begin)
+        ipc, off = h.hadpsgd_peer_ipc_export()
+        mine = torch.tensor(list(ipc) + list(off.to_bytes(8, "little")), dtype=torch.uint8)
+        got = [torch.empty_like(mine) for _ in range(world)]
+        dist.all_gather(got, mine)
+        for r in range(world):
+            if r != rank:
+                raw = bytes(got[r].tolist())
+                h.hadpsgd_peer_ipc_attach(r, raw[:64], int.from_bytes(raw[64:], "little"))
+        for s in range(4):
+            device.fill(h.hadpsgd_weights(s)[:P], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, lo + s, 0), "normal", 0.05)
+        for k in range(steps):
+            for s in range(4):
+                for g in range(G):
+                    device.fill(h.hadpsgd_grads(s, g)[:P], gen.stream_key(seed, gen.STREAM_GRAD, k, lo + s, g), "normal", 1e-3)
+            h.hadpsgd_step(0.1, 0.9, k)
+            torch.cuda.synchronize()
+            dist.barrier()                              # epoch barrier
+        h.hadpsgd_peer_flush()
+        torch.cuda.synchronize()
+        dist.barrier()                                  # nobody tears its stage region down before all have read it
+        w = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(4)])
+        v = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(4)])
+        np.savez(os.path.join(out_dir, f"rank{rank}.npz"), w=w, v=v)
+        dist.barrier()
+        h.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(600)
+def test_peer_partition_two_processes_cuda_ipc(H, oracle_mod, tmp_path):
+    """The cross-process plumbing of bench.py --partition superlearner, on one GPU: two processes, each
+    owning 4 of 8 super-learners, read each other's stage buffers through cudaIpcOpenMemHandle
+    mappings inside the fused kernel.  Bit-exact against the oracle on all 8."""
+    import socket
+    import torch.multiprocessing as mp
+    from fixtures import problem
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    mp.spawn(_ipc_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    S, G, P, seed, steps = 8, 2, 200_003, 431, 5
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    for k in range(steps):
+        oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k)
+    parts = [np.load(tmp_path / f"rank{r}.npz") for r in range(2)]
+    assert np.array_equal(bits(np.concatenate([p["w"] for p in parts])), bits(ow))
+    assert np.array_equal(bits(np.concatenate([p["v"] for p in parts])), bits(ov))
+
+
 # ------------------------------------------------------------------------------- API behaviour
 
 def test_custom_matching_and_unpaired(H, oracle_mod):
