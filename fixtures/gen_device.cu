@@ -51,7 +51,14 @@ extern "C" int hadpsgd_fixture_fill(void* dev_out, long long n, long long elem_o
                                     float scale, int dist, int out_bf16, void* stream) {
     if (n <= 0) return 0;
     long long blocks = (n + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    static int cap = 0;                      // 16 blocks per SM of the current device
+    if (cap == 0) {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
+            sms = 128;
+        cap = sms * 16;
+    }
+    if (blocks > cap) blocks = cap;
     fill_kernel<<<static_cast<unsigned>(blocks), 256, 0, static_cast<cudaStream_t>(stream)>>>(
         dev_out, n, elem_offset, key, scale, dist, out_bf16);
     return static_cast<int>(cudaGetLastError());

@@ -112,7 +112,6 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
     a.lr = lr; a.mu = mu;
     a.invG = 1.0f / static_cast<float>(h->L.G);   // fp32 reciprocal, exact for G = 1,2,4,8 (R5)
     a.accumulate_diag = accumulate ? 1 : 0;
-    a.tile_major = wmode == kSlots ? 1 : 0;
     a.S = h->L.S;
     a.partials = h->d_partials; a.diag = h->d_diag; a.ticket = h->d_ticket;
     for (int j = 0; j < n_items; ++j) {
@@ -125,7 +124,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
 
     // per-warp diagnostic accumulators [warps][items][quantities]; the last block's column sums reuse
     // the buffer and need max(threads, rows) doubles.  At most 18 KB: no opt-in needed.
-    const int nq = wmode == kPeer ? kNQPeer : kNQ;
+    const int nq = plan.wmode == kPeer ? kNQPeer : kNQ;
     size_t smem = 0;
     if (diag) {
         size_t cells = static_cast<size_t>(plan.threads / 32) * n_items * nq;
@@ -143,22 +142,21 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
     int bps = h->blocks_per_sm > 0 ? h->blocks_per_sm : plan.blocks_per_sm;
     if (bps > occ) bps = occ;                      // persistent grid: never more than fit at once
     long long n_units = a.unit_end - a.unit_begin;
-    long long want = (n_units + plan.tile_units - 1) / plan.tile_units * a.n_work;   // (item, tile) pairs
+    const long long n_tiles = (n_units + plan.tile_units - 1) / plan.tile_units;
+    // shared slots: a block owns whole tiles (and walks every item of each); else (item, tile) pairs
+    long long want = plan.wmode == kChain ? n_tiles : n_tiles * a.n_work;
     long long grid = static_cast<long long>(h->num_sms) * bps;
     if (grid > want) grid = want;
     if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;
     if (grid < 1) grid = 1;
-
-    {   // how many blocks work on any one item (the last block sums exactly their partials)
-        const long long n_tiles = (n_units + plan.tile_units - 1) / plan.tile_units;
-        long long per = grid;
-        if (a.tile_major) {
-            long long x = a.n_work, y = grid;
-            while (y) { const long long t = x % y; x = y; y = t; }   // x = gcd(n_work, grid)
-            per = grid / x;
-        }
-        a.touch_count = static_cast<int>(n_tiles < per ? n_tiles : per);
+    // how many blocks work on any one item (the last block sums exactly their partials)
+    long long per = grid;
+    if (plan.wmode == kSlots) {                      // tile-major walk: blocks (i * n_work + j) mod grid
+        long long x = a.n_work, y = grid;
+        while (y) { const long long t = x % y; x = y; y = t; }   // x = gcd(n_work, grid)
+        per = grid / x;
     }
+    a.touch_count = static_cast<int>(plan.wmode == kChain ? grid : (n_tiles < per ? n_tiles : per));
     void* params[] = {&a};
     CUDA_TRY(h, cudaLaunchKernel(plan.fn, dim3(static_cast<unsigned>(grid)), dim3(plan.threads), params, smem, h->stream));
     h->launches++;

@@ -8,7 +8,7 @@
 
 namespace hadpsgd {
 
-struct LaunchPlan { const void* fn; int threads; int tile_units; int blocks_per_sm; };
+struct LaunchPlan { const void* fn; int threads; int tile_units; int blocks_per_sm; int wmode; };
 
 // wmode: kOwn | kSlots (kPair only) | kPeer (kPair and kSingle, no bf16 working copy).  A
 // combination that is not instantiated returns fn == nullptr.
@@ -22,7 +22,7 @@ LaunchPlan plan_bf16_emit(int G, bool exact, bool diag, int mode, int wmode);
 // warps than that measured slower on this path (more DRAM pages open at once).
 template <int G, bool BF16, bool EXACT, bool DIAG, int MODE, bool EMIT, int WMODE>
 LaunchPlan plan_for() {
-    static_assert(WMODE != kSlots || MODE == kPair, "slots are shared by the members of a kPair item only");
+    static_assert((WMODE != kSlots && WMODE != kChain) || MODE == kPair, "slots are shared by the members of a kPair item only");
     static_assert(kInlineItems == kMaxItemsPerLaunch, "host and kernel disagree on the items per launch");
     constexpr int members = (MODE == kSingle) ? 1 : 2;
     constexpr int loads_per_unit = members * ((G > 0 ? G : 4) + (BF16 ? 4 : 2));
@@ -39,12 +39,14 @@ LaunchPlan plan_for() {
     constexpr int in_flight = THREADS * U * loads_per_unit * 32;           // bytes per block
     constexpr int BPS = in_flight >= 48 * 1024 ? 1 : 2;
     return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, EMIT, WMODE, U, THREADS, 1>),
-            THREADS, THREADS * U, BPS};
+            THREADS, THREADS * U, BPS, WMODE};
 }
 
 template <int G, bool BF16, bool EXACT, bool DIAG, bool EMIT>
 LaunchPlan pick_mode(int mode, int wmode) {
-    const LaunchPlan none = {nullptr, 0, 0, 0};
+    const LaunchPlan none = {nullptr, 0, 0, 0, 0};
+    // shared slots: the CHAIN walk where it measured faster (<= 12 loads per pair unit: fp32 G <= 4)
+    constexpr bool chain = !BF16 && G >= 1 && G <= 4;
     if (wmode == kPeer) {
         if constexpr (EMIT) return none;
         else {
@@ -54,7 +56,7 @@ LaunchPlan pick_mode(int mode, int wmode) {
         }
     }
     switch (mode) {
-        case kPair: return wmode == kSlots ? plan_for<G, BF16, EXACT, DIAG, kPair, EMIT, kSlots>()
+        case kPair: return wmode == kSlots ? plan_for<G, BF16, EXACT, DIAG, kPair, EMIT, chain ? kChain : kSlots>()
                                            : plan_for<G, BF16, EXACT, DIAG, kPair, EMIT, kOwn>();
         case kSingle: return plan_for<G, BF16, EXACT, DIAG, kSingle, EMIT, kOwn>();
         default: return wmode == kOwn ? plan_for<G, BF16, EXACT, DIAG, kPairEq7, EMIT, kOwn>() : none;

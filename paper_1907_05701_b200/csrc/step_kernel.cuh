@@ -42,7 +42,8 @@ enum Mode : int { kPair = 0, kSingle = 1, kPairEq7 = 2 };
 // kOwn: member s reads and writes weight buffer s.  kSlots: read buffer a, write buffer o (pair
 // members may share one buffer: HADPSGD_SHARE_PAIR_WEIGHTS).  kPeer: a, o and the pending-mix
 // partner buffer b (super-learner partition over several arenas / GPUs).
-enum WMode : int { kOwn = 0, kSlots = 1, kPeer = 2 };
+// kChain: kSlots with the CHAIN walk (below); the dispatcher picks it for the kernels it measured faster on.
+enum WMode : int { kOwn = 0, kSlots = 1, kPeer = 2, kChain = 3 };
 
 // Work item: super-learner indices s, p of the pair inside THIS handle (momentum and gradients
 // are always the member's own buffers); a_*: weight buffer index read; o_*: weight buffer index
@@ -67,7 +68,6 @@ struct StepArgs {
     int n_work;
     int S;
     int accumulate_diag;  // 0: diag = result ; 1: diag += result (chunked host path)
-    int tile_major;       // 0: item-major walk ; 1: tile-major (shared slots: L2 reuse)
     int touch_count;      // blocks that work on any one item (host: from n_tiles, grid, walk order)
     float lr, mu, invG;
     Item items[kInlineItems];
@@ -293,7 +293,8 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     // weights addressed through the item's buffer indices: shared pairs, peer mode, and every
     // unmixed item (after an un-sharing copy the buffer of an unmixed member need not be its own)
     constexpr bool SLOTS = WMODE != kOwn || MODE == kSingle;
-    constexpr bool ONE_STORE = (WMODE == kSlots);   // pair members share ONE output buffer
+    static_assert(WMODE != kChain || MODE == kPair, "the CHAIN walk is for shared pair slots");
+    constexpr bool ONE_STORE = (WMODE == kSlots || WMODE == kChain);   // pair members share ONE output buffer
     constexpr int NP = PAIRED ? U : 1;   // array extent of the partner's registers
     constexpr int WARPS = THREADS / 32;
     constexpr int NQ = PEER ? kNQPeer : kNQ;
@@ -315,9 +316,9 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     // Flattened (work item, tile) space; block b takes global tiles b, b+grid, ...
     //  item-major: tiles of item 0, then item 1, ...: for large P the whole chip streams one pair
     //              at a time (few 2 MB pages and DRAM rows live at once).
-    //  tile-major: all items of tile 0, then tile 1, ...: used when pairs share weight slots --
-    //              the slot two neighbouring pairs both read is then fetched from HBM once and
-    //              hits in L2 the second time.
+    //  tile-major (pairs share weight slots): all items of tile 0, then tile 1, ...: the slot two
+    //              neighbouring pairs both read is fetched from HBM once and hits in L2 the second time.
+    //  CHAIN (ditto): block b takes TILES b, b+grid, ... and walks every item of a tile itself -- see below.
     const long long n_tiles = (n_units + TILE - 1) / TILE;
     const long long total_tiles = n_tiles * a.n_work;
     // a5: per-thread sums of the item being worked on; when the block moves to another item they
@@ -349,13 +350,35 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
         d_gs = d_gp = d_ws = d_wp = d_gap = 0.;
         d_pws = d_pwp = d_pgs = d_pgp = 0.;
     };
-    for (long long gt = blockIdx.x; gt < total_tiles; gt += gridDim.x) {
+    // CHAIN (shared slots): the block owns whole tiles and walks ALL items of a tile in order, so the
+    // weight vector item j read for its second member -- which, in the ring schedule, is the very
+    // slot item j+1 reads for its first member -- is handed on in registers, and the slot the last
+    // item shares with the first is kept from the first: every shared slot is fetched ONCE.
+    // (Measured on the 16 x 4 fp32 configs: 1.5 % faster and DRAM reads at the mode's own byte model; on
+    // the 8 x 8 configs, where weights are a small share of the reads and the carry costs 16-32 more
+    // registers, the plain tile-major walk -- all items of tile 0 across neighbouring blocks, then tile
+    // 1, ..., the shared slot hitting in L2 -- stays 1-1.5 % faster, so both exist.)
+    constexpr bool CHAIN = (WMODE == kChain);
+    constexpr bool TILE_MAJOR = (WMODE == kSlots);
+    Vec<UNIT> carry[CHAIN ? U : 1], first_w[CHAIN ? U : 1];
+    int prev_ap = -1, first_as = -1;
+    long long seq = 0;                                   // CHAIN: position in this block's (tile, item) walk
+    for (long long gt = blockIdx.x; ; gt += gridDim.x, ++seq) {
         int j;
         long long tile;
-        if (WMODE == kSlots && a.tile_major) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
-        else { j = static_cast<int>(gt / n_tiles); tile = gt - static_cast<long long>(j) * n_tiles; }
+        if constexpr (CHAIN) {
+            const long long round = seq / a.n_work;
+            j = static_cast<int>(seq - round * a.n_work);
+            tile = blockIdx.x + round * gridDim.x;
+            if (tile >= n_tiles) break;
+        } else {
+            if (gt >= total_tiles) break;
+            if constexpr (TILE_MAJOR) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
+            else { j = static_cast<int>(gt / n_tiles); tile = gt - static_cast<long long>(j) * n_tiles; }
+        }
         const long long base = tile * TILE;
-        if (j != cur) {                                  // block-uniform
+        bool take_carry = false, take_first = false;     // CHAIN: w_s / w_p already sit in registers
+        if (j != cur || CHAIN) {                         // block-uniform
             if constexpr (DIAG) { if (cur >= 0) hand_over(cur); }
             cur = j;
             touched |= 1u << j;
@@ -366,6 +389,12 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             if constexpr (PEER) {
                 pb_s = it.b_s ? a.peer[it.b_s - 1] : nullptr;
                 pb_p = (PAIRED && it.b_p) ? a.peer[it.b_p - 1] : nullptr;
+            }
+            if constexpr (CHAIN) {
+                take_carry = j > 0 && it.a_s == prev_ap;
+                take_first = j > 0 && j == a.n_work - 1 && it.a_p == first_as;
+                if (j == 0) first_as = it.a_s;
+                prev_ap = it.a_p;
             }
         }
         {
@@ -388,10 +417,12 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     if (live[q]) {
                         load_grads<GA, BF16>(gbytes, P, o_gs + elem[q], grs[q]);
                         if constexpr (PAIRED) load_grads<GA, BF16>(gbytes, P, o_gp + elem[q], grp[q]);
-                        load_state<UNIT>(a.w, (SLOTS ? o_ws : o_vs) + elem[q], ws[q]);
+                        if (CHAIN && take_carry) ws[q] = carry[q];
+                        else load_state<UNIT>(a.w, (SLOTS ? o_ws : o_vs) + elem[q], ws[q]);
                         load_state<UNIT>(a.v, o_vs + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
+                            if (CHAIN && take_first) wp[q] = first_w[q];
+                            else load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
                             load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
                         if constexpr (PEER) {
@@ -411,10 +442,12 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
                 for (int q = 0; q < U; ++q) {
                     if (live[q]) {
-                        load_state<UNIT>(a.w, (SLOTS ? o_ws : o_vs) + elem[q], ws[q]);
+                        if (CHAIN && take_carry) ws[q] = carry[q];
+                        else load_state<UNIT>(a.w, (SLOTS ? o_ws : o_vs) + elem[q], ws[q]);
                         load_state<UNIT>(a.v, o_vs + elem[q], vs[q]);
                         if constexpr (PAIRED) {
-                            load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
+                            if (CHAIN && take_first) wp[q] = first_w[q];
+                            else load_state<UNIT>(a.w, (SLOTS ? o_wp : o_vp) + elem[q], wp[q]);
                             load_state<UNIT>(a.v, o_vp + elem[q], vp[q]);
                         }
                         if constexpr (PEER) {
@@ -427,6 +460,13 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                 }
             }
 
+            if constexpr (CHAIN) {       // the OLD weights, as read, travel on (dead lanes carry junk they never use)
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    if (j == 0) first_w[q] = ws[q];
+                    carry[q] = wp[q];
+                }
+            }
 #pragma unroll
             for (int q = 0; q < U; ++q) {
                 const long long os = o_vs + elem[q];
@@ -552,23 +592,23 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
         if (!s_last) return;
         __threadfence();
         // Item j was worked on by exactly touch_count blocks: the i-th of them (in tile order) is block
-        // (j * n_tiles + i) mod grid in the item-major walk, (i * n_work + j) mod grid in the tile-major
-        // one.  Only their partials are read (for a small problem that is one block per tile instead of
+        // (j * n_tiles + i) mod grid in the item-major walk; in the CHAIN walk it is every block.  Only their partials are read (for a small problem that is one block per tile instead of
         // the whole grid), with every thread busy: thread (c, row) sums contributors c, c+C, c+2C, ... of
         // its row (independent loads), then the C column sums of a row are added in order.  The result
         // depends on the launch shape only: run-to-run deterministic.
         const int C = (THREADS / R) > 0 ? (THREADS / R) : 1;
         double* s_col = s_acc;           // reuse: C x R <= max(THREADS, R) doubles (the host sizes it)
         const unsigned nb = gridDim.x;
-        const bool tmaj = (WMODE == kSlots) && a.tile_major;
-        // contributor i of item j is block (first + i * step) mod nb; walked incrementally (no division
-        // inside the loop)
-        const unsigned step1 = tmaj ? static_cast<unsigned>(a.n_work) % nb : 1u % nb;
+        // contributor i of item j is block (first + i * step1) mod nb; walked incrementally (no division
+        // inside the loop).  Item-major: first = j * n_tiles, step 1.  Tile-major: first = j, step n_work.
+        // CHAIN: every block works on every item.
+        const unsigned step1 = TILE_MAJOR ? static_cast<unsigned>(a.n_work) % nb : 1u % nb;
         const unsigned stepC = static_cast<unsigned>((static_cast<unsigned long long>(step1) * C) % nb);
         for (int task = tid; task < R * C; task += THREADS) {
             const int c = task / R, row = task - c * R;
             const unsigned j = row / NQ;
-            const unsigned long long first = tmaj ? j : static_cast<unsigned long long>(j) * static_cast<unsigned long long>(n_tiles);
+            const unsigned long long first = CHAIN ? 0ull : TILE_MAJOR ? static_cast<unsigned long long>(j)
+                                                   : static_cast<unsigned long long>(j) * static_cast<unsigned long long>(n_tiles);
             unsigned b = static_cast<unsigned>((first + static_cast<unsigned long long>(step1) * c) % nb);
             double sum = 0.;
 #pragma unroll 4
