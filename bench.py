@@ -36,6 +36,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+_REAL_STDOUT = None
 METRIC = "learner_params_updated_per_sec"
 UNIT = "learner-params/s"
 LR, MU = 0.1, 0.9
@@ -93,6 +94,9 @@ def parse_args():
                     help="also write the bf16 working copy of the weights every step (row f2; +2 B/param)")
     ap.add_argument("--partition", default="range", choices=["range", "superlearner", "weak"],
                     help="how N > 1 GPUs share the work (ignored for N = 1)")
+    ap.add_argument("--emulate-ranks", type=int, default=0,
+                    help="N = 1 only: time the super-learner partition over R HADPSGD_PEER handles on ONE GPU (one stream; "
+                         "peer reads are local HBM reads) -- kernel cost of the partition, not an NVLink measurement")
     ap.add_argument("--no-ceiling", action="store_true", help="skip the pure-read / pure-write membench legs")
     ap.add_argument("--cpu-repeats", type=int, default=3)
     ap.add_argument("--sweep", action="store_true",
@@ -422,14 +426,16 @@ def make_problem(H, torch, dist, args, cfg, flags, local, rank, world):
     S, G, P = cfg["S"], cfg["G"], cfg["P"]
     gdt = H.BF16 if cfg["grad"] == "bf16" else H.F32
     wdt = H.BF16 if args.emit_bf16 else H.F32
-    part = args.partition if world > 1 else "single"
+    # N = 1: one plain handle, unless launched by torch.distributed.run with an explicit partition (a
+    # one-rank smoke test of the partition's plumbing)
+    part = args.partition if (world > 1 or (dist is not None and args.partition == "superlearner")) else "single"
     dist_name = cfg["dist"]
     if part in ("single", "weak"):
         h = H.Hadpsgd(S, G, cfg["seg_len"], gdt, flags, device=local, working_dtype=wdt)
         seed = 2000 + rank            # weak: every rank is its own problem
         problem.fill_weights(h, seed)
         problem.fill_grads(h, seed, 0, dist_name)
-        info = {"units": S * G * P, "scaling": "weak",
+        info = {"units": S * G * P, "scaling": "weak", "partition": part,
                 "parallelism": "single GPU" if world == 1 else f"weak: {world} independent problems of the configured size, no collective"}
         return h, info
     if part == "range":
@@ -445,7 +451,7 @@ def make_problem(H, torch, dist, args, cfg, flags, local, rank, world):
             for g_ in range(G):
                 device.fill(h.hadpsgd_grads(s_, g_)[:hi - lo], gen.stream_key(seed, gen.STREAM_GRAD, 0, s_, g_), dist_name, 1e-3,
                             elem_offset=lo)
-        info = {"units": S * G * (hi - lo), "scaling": "strong", "shard": [lo, hi],
+        info = {"units": S * G * (hi - lo), "scaling": "strong", "shard": [lo, hi], "partition": part,
                 "parallelism": f"range: one {P}-parameter model, rank r owns hadpsgd_shard_range(P, {world}, r) of every buffer; "
                                "no data-path collective (diagnostics all-reduced after the timed region)"}
         return h, info
@@ -479,7 +485,7 @@ def make_problem(H, torch, dist, args, cfg, flags, local, rank, world):
     # odd (or even) step and reads its partner's 4*P bytes at the next launch
     strad = [sum(1 for sg in range(rank_begin[rank], rank_begin[rank + 1])
                  if not rank_begin[rank] <= H.hadpsgd_pairing(S, k)[sg] < rank_begin[rank + 1]) for k in (0, 1)]
-    info = {"units": S_l * G * P, "scaling": "strong", "barrier": True,
+    info = {"units": S_l * G * P, "scaling": "strong", "barrier": True, "partition": part,
             "nvlink_read_bytes_per_rank_per_step": [strad[1] * 4 * P, strad[0] * 4 * P],   # [even step reads what the odd step left, odd step ...]
             "parallelism": f"superlearner: rank r owns super-learners [{S_l}r, {S_l}(r+1)) of {S}; straddling pairs mixed by peer reads "
                            f"of the partner's stage buffer inside the fused kernel (CUDA IPC); epoch barrier = 1-element NCCL all-reduce per step"}
@@ -535,8 +541,21 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
+    # The oracle baseline first, in a process that has not touched CUDA yet: with a CUDA context and tens
+    # of GB of pinned host memory mapped, the same single-threaded oracle runs 1.6 x slower (its 268 MB
+    # scratch vector is allocated and faulted in every step) -- measured as it stands either way, but the
+    # clean process is the fairer baseline and is what --impl reference sees too.
+    cpu_line = None
+    if world == 1 and rank == 0 and not args.no_cpu_baseline:
+        cpu_line = cpu_baseline(workload(args.workload), args.cpu_sample_elems, args.cpu_sample_steps, args.cpu_repeats)
     dist = None
     if world > 1 or "RANK" in os.environ:          # launched by torch.distributed.run (any N)
+        # stdout carries the one JSON line only: NCCL prints its version banner to fd 1, so fd 1 is
+        # pointed at stderr for the rest of the run and the line goes out through a saved copy
+        global _REAL_STDOUT
+        sys.stdout.flush()
+        _REAL_STDOUT = os.fdopen(os.dup(1), "w")
+        os.dup2(2, 1)
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world} (launch N>1 with torch.distributed.run)"
@@ -585,7 +604,7 @@ def run_ours(args):
         units = float(t_units[0])
         if e2e:
             e2e = (sharding.max_over_ranks(e2e[0], dist, "cuda"),) + e2e[1:]
-        if diag is not None and args.partition == "range" and world > 1:
+        if diag is not None and info.get("partition") == "range":
             # the only collective of the range partition: 3*S doubles, outside the timed region
             diag = sharding.allreduce_diagnostics(diag, dist, "cuda")
     arena_bytes = h.arena_bytes
@@ -600,7 +619,7 @@ def run_ours(args):
     # results; one weight write per pair and one HBM fetch of the buffer two pairs read).
     shared = None
     can_share = (not (flags & (H.NO_MIX | H.EQ7_LITERAL | H.SHARE_PAIR_WEIGHTS)) and S > 1 and S % 2 == 0
-                 and (world == 1 or args.partition == "weak"))
+                 and info.get("partition") in ("single", "weak"))
     if can_share and not args.no_share_leg:
         from fixtures import problem
         hs = H.Hadpsgd(S, G, cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, flags | H.SHARE_PAIR_WEIGHTS,
@@ -623,7 +642,7 @@ def run_ours(args):
         per_sp = cfg["G"] * cfg["b_g"] + 16 + (2 if cfg.get("emit") else 0)        # bytes per super-learner-parameter
         abytes_rank = S_rank * P_rank * per_sp                                      # algorithmic bytes of ONE launch (this rank)
         achieved = abytes_rank / t_step / 1e9
-        traffic, traffic_src = (None, "n/a: per-rank launch of a partition") if world > 1 else \
+        traffic, traffic_src = (None, "n/a: per-rank launch of a partition") if info.get("partition") != "single" else \
             ncu_traffic(args.workload, args.flags, args.emit_bf16)
         roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_src,
@@ -645,7 +664,7 @@ def run_ours(args):
                        "working_dtype": "bf16" if args.emit_bf16 else "f32", "lr": LR, "momentum": MU,
                        "resident_bytes_per_gpu": arena_bytes, "flags": args.flags or "default (diagnostics on)",
                        "l2": "inputs larger than L2 (working set per step >> 126 MB); no flush needed",
-                       "partition": args.partition if world > 1 else "single", "parallelism": info["parallelism"]},
+                       "partition": info.get("partition", "single"), "parallelism": info["parallelism"]},
             "roofline": roof, "clocks": clocks, "gpu_launches": launches,
         }
         for k_ in ("shard", "nvlink_read_bytes_per_rank_per_step"):
@@ -675,12 +694,85 @@ def run_ours(args):
                                    f"buffers (PCIe Gen5 x16, {PCIE_GEN5_X16_GBS:.0f} GB/s nominal per direction), which the "
                                    "fused kernel overlaps chunk by chunk; the new weights and momenta stay resident in HBM "
                                    "(the learners live on the GPU), so the device-to-host traffic is the diagnostics only"}
-        if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg, args.cpu_sample_elems, args.cpu_sample_steps, args.cpu_repeats)
-        print(json.dumps(line), flush=True)
+        if cpu_line is not None:
+            line["cpu_baseline"] = cpu_line
+        print(json.dumps(line), file=_REAL_STDOUT or sys.stdout, flush=True)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def run_emulated_partition(args):
+    """--emulate-ranks R: the super-learner partition of the workload over R PEER handles on
+    one GPU and one stream.  A step = the step of every handle.  Even and odd ring steps differ (odd steps
+    publish u, even steps resolve the pending mixes), so they are timed separately; `value` uses their mean."""
+    import torch
+    import paper_1907_05701_b200 as H
+    from fixtures import device, generator as gen
+    H.lib()
+    torch.cuda.set_device(0)
+    cfg = workload(args.workload)
+    S, G, P, R = cfg["S"], cfg["G"], cfg["P"], args.emulate_ranks
+    assert S % R == 0 and len(cfg["seg_len"]) == 1, "--emulate-ranks needs S divisible by R and a flat workload"
+    S_l = S // R
+    rb = [r * S_l for r in range(R + 1)]
+    gdt = H.BF16 if cfg["grad"] == "bf16" else H.F32
+    hs = [H.Hadpsgd(S_l, G, cfg["seg_len"], gdt, parse_flags(H, args.flags) | H.PEER, device=0) for _ in range(R)]
+    for r, h in enumerate(hs):
+        h.hadpsgd_peer_init(r, R, rb)
+    for r, h in enumerate(hs):
+        for q, other in enumerate(hs):
+            if q != r:
+                h.hadpsgd_peer_attach(q, other.hadpsgd_peer_stage())
+        for s_ in range(S_l):
+            device.fill(h.hadpsgd_weights(s_), gen.stream_key(2000, gen.STREAM_WEIGHT, 0, rb[r] + s_, 0), "normal", 0.05)
+            for g_ in range(G):
+                device.fill(h.hadpsgd_grads(s_, g_), gen.stream_key(2000, gen.STREAM_GRAD, 0, rb[r] + s_, g_), cfg["dist"], 1e-3)
+    torch.cuda.synchronize()
+    k = 0
+    for _ in range(max(args.warmup, 3) // 2 * 2 + 2):
+        for h in hs:
+            h.hadpsgd_step(LR, MU, k)
+        k += 1
+    torch.cuda.synchronize()
+    n0 = sum(h.hadpsgd_launch_count() for h in hs)
+    sampler = ClockSampler(0)
+    sampler.start()
+    per = {0: [], 1: []}
+    for _ in range(args.steps):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for h in hs:
+            h.hadpsgd_step(LR, MU, k)
+        ev1.record()
+        torch.cuda.synchronize()
+        per[k % 2].append(ev0.elapsed_time(ev1) / 1e3)
+        k += 1
+    clocks = sampler.stop()
+    launches = sum(h.hadpsgd_launch_count() for h in hs) - n0
+    even, odd = sum(per[0]) / max(len(per[0]), 1), sum(per[1]) / max(len(per[1]), 1)
+    t_step = (sum(per[0]) + sum(per[1])) / args.steps
+    pending_even = sum(1 for sg in range(S) if H.hadpsgd_pairing(S, 1)[sg] // S_l != sg // S_l)   # left pending by odd steps
+    abytes = algorithmic_bytes(cfg)
+    peak, peak_src = measured_peak()
+    for h in hs:
+        h.close()
+    line = {"metric": METRIC, "value": S * G * P / t_step, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": args.workload, "S": S, "G": G, "P": P, "partition": "superlearner (emulated)", "emulated_ranks": R,
+                       "parallelism": f"{R} HADPSGD_PEER handles ({S_l} super-learners each) on ONE GPU and one stream: the kernels of "
+                                      "the partition with peer reads served from local HBM; NOT an NVLink measurement",
+                       "ms_even_step": even * 1e3, "ms_odd_step": odd * 1e3,
+                       "stage_bytes_read_per_even_step": pending_even * 4 * P,
+                       "note": "odd ring steps: straddling members publish u (same bytes as a plain step); even steps: every pending "
+                               "member also reads its partner's stage buffer (4 B per parameter on top of the algorithmic bytes)"},
+            "roofline": {"bound": "hbm", "achieved": abytes / t_step / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": abytes / t_step / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": abytes, "frac_of_8TBps_nominal": abytes / t_step / 1e9 / 8000.0,
+                         "achieved_even_step_incl_stage_reads": (abytes + pending_even * 4 * P) / even / 1e9 if even else None},
+            "clocks": clocks, "gpu_launches": launches}
+    print(json.dumps(line), flush=True)
 
 
 def run_sweep(args):
@@ -753,6 +845,8 @@ def main():
     args = parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.emulate_ranks and args.impl == "ours":
+        run_emulated_partition(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

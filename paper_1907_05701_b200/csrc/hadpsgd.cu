@@ -86,13 +86,13 @@ struct DeviceGuard {
 
 bool is_peer(const hadpsgd_ctx* h) { return (h->flags & HADPSGD_PEER) != 0; }
 
-int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, bool shared_slots, float lr, float mu,
+int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, int wmode_req, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
     const bool exact = h->flags & HADPSGD_DETERMINISTIC;
     const bool diag = !(h->flags & HADPSGD_NO_DIAG);
     const bool emit = h->L.working_dtype == HADPSGD_BF16;
-    const int wmode = is_peer(h) ? kPeer : ((shared_slots && mode == kPair) ? kSlots : kOwn);
+    const int wmode = (wmode_req == kSlots && mode != kPair) ? kOwn : wmode_req;
     LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode, wmode) : plan_f32_emit(h->L.G, exact, diag, mode, wmode))
                            : (bf16 ? plan_bf16(h->L.G, exact, diag, mode, wmode) : plan_f32(h->L.G, exact, diag, mode, wmode));
     if (!plan.fn) { h->err = "this combination of flags has no kernel"; return HADPSGD_INVALID_ARG; }
@@ -165,12 +165,12 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, b
 
 // All items of one mode over [elem_begin, elem_end); more than kInlineItems items (S > 64 paired or
 // S > 32 unmixed super-learners) take several launches.
-int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, bool shared_slots, float lr, float mu,
+int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, int wmode, float lr, float mu,
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     if (elem_end <= elem_begin) return HADPSGD_OK;
     for (size_t first = 0; first < items.size(); first += kInlineItems) {
         const int n = static_cast<int>(items.size() - first < static_cast<size_t>(kInlineItems) ? items.size() - first : kInlineItems);
-        int rc = launch_chunk(h, items.data() + first, n, mode, shared_slots, lr, mu, elem_begin, elem_end, accumulate);
+        int rc = launch_chunk(h, items.data() + first, n, mode, wmode, lr, mu, elem_begin, elem_end, accumulate);
         if (rc != HADPSGD_OK) return rc;
     }
     return HADPSGD_OK;
@@ -180,11 +180,29 @@ int launch_items(hadpsgd_ctx* h, const std::vector<WorkItem>& items, int mode, b
 int step_range(hadpsgd_ctx* h, const StepPlan& sp, float lr, float mu, int64_t elem_begin, int64_t elem_end,
                bool accumulate) {
     const int pair_mode = (h->flags & HADPSGD_EQ7_LITERAL) ? kPairEq7 : kPair;
-    int rc = launch_items(h, sp.pairs, pair_mode, sp.shared, lr, mu, elem_begin, elem_end, accumulate);
-    if (rc != HADPSGD_OK) return rc;
-    // unmixed super-learners (S == 1, NO_MIX, or partner[s] == s in a custom matching), and in peer mode
-    // the members that publish u for a partner in another arena
-    return launch_items(h, sp.singles, kSingle, false, lr, mu, elem_begin, elem_end, accumulate);
+    if (!is_peer(h)) {
+        int rc = launch_items(h, sp.pairs, pair_mode, sp.shared ? kSlots : kOwn, lr, mu, elem_begin, elem_end, accumulate);
+        if (rc != HADPSGD_OK) return rc;
+        // unmixed super-learners (S == 1, NO_MIX, or partner[s] == s in a custom matching)
+        return launch_items(h, sp.singles, kSingle, kOwn, lr, mu, elem_begin, elem_end, accumulate);
+    }
+    // Peer mode.  Only items that first have to resolve a pending mix need the kPeer kernel (two more
+    // loads per member, more registers).  A pair without one reads and writes its members' main
+    // buffers -- exactly the kOwn pair kernel -- and a single without one (unmixed, or publishing u for
+    // a partner in another arena) is the ordinary kSingle kernel, which addresses weights through the
+    // item's buffer indices anyway.  The plain kernels do not know pend_wsq / pend_gap: clear them.
+    if (!(h->flags & HADPSGD_NO_DIAG) && !accumulate)
+        CUDA_TRY(h, cudaMemsetAsync(h->d_diag + 3 * h->L.S, 0, sizeof(double) * 2 * h->L.S, h->stream));
+    std::vector<WorkItem> part[2][2];   // [pairs | singles][plain | pending]
+    for (const WorkItem& it : sp.pairs) part[0][(it.b_s || it.b_p) ? 1 : 0].push_back(it);
+    for (const WorkItem& it : sp.singles) part[1][it.b_s ? 1 : 0].push_back(it);
+    for (int kind = 0; kind < 2; ++kind)
+        for (int pend = 0; pend < 2; ++pend) {
+            int rc = launch_items(h, part[kind][pend], kind == 0 ? kPair : kSingle, pend ? kPeer : kOwn, lr, mu,
+                                  elem_begin, elem_end, accumulate);
+            if (rc != HADPSGD_OK) return rc;
+        }
+    return HADPSGD_OK;
 }
 
 // Copies weight slot src to slot dst (and the bf16 working copy with it) on the handle's stream.
