@@ -528,6 +528,49 @@ def test_peer_partition_two_processes_cuda_ipc(H, oracle_mod, tmp_path):
     assert np.array_equal(bits(np.concatenate([p["v"] for p in parts])), bits(ov))
 
 
+def test_range_partition_shards_equal_the_unsharded_model(H, oracle_mod, torch_cuda):
+    """bench.py --partition range: rank r owns hadpsgd_shard_range(P, N, r) of every buffer of ONE model.
+    Three shard handles on one GPU, filled from the GLOBAL element index, must reproduce the unsharded
+    handle bit for bit, and their diagnostics must add up to its diagnostics (the all-reduce)."""
+    torch = torch_cuda
+    from fixtures import device, generator as gen, problem
+    S, G, P, seed, world = 4, 2, 64 * 3001, 501, 3
+    full = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
+    problem.fill_weights(full, seed)
+    shards = []
+    for r in range(world):
+        lo, hi = H.hadpsgd_shard_range(P, world, r)
+        h = H.Hadpsgd(S, G, [hi - lo], H.F32, H.DETERMINISTIC)
+        for s in range(S):
+            device.fill(h.hadpsgd_weights(s)[:hi - lo], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, s, 0), "normal", 0.05, elem_offset=lo)
+        shards.append((lo, hi, h))
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    for k in range(3):
+        problem.fill_grads(full, seed, k)
+        full.hadpsgd_step(LR, MU, k)
+        od = oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k, diag=True)
+        tot = {n: np.zeros(S) for n in ("gsq", "wsq", "gap")}
+        for lo, hi, h in shards:
+            for s in range(S):
+                for g in range(G):
+                    device.fill(h.hadpsgd_grads(s, g)[:hi - lo], gen.stream_key(seed, gen.STREAM_GRAD, k, s, g), "normal", 1e-3,
+                                elem_offset=lo)
+            h.hadpsgd_step(LR, MU, k)
+            d = h.hadpsgd_diagnostics()
+            for n in tot:
+                tot[n] += d[n]
+        assert_diag(tot, od, k)
+    torch.cuda.synchronize()
+    for lo, hi, h in shards:
+        for s in range(S):
+            assert torch.equal(h.hadpsgd_weights(s)[:hi - lo], full.hadpsgd_weights(s)[lo:hi])
+            assert torch.equal(h.hadpsgd_momentum(s)[:hi - lo], full.hadpsgd_momentum(s)[lo:hi])
+        h.close()
+    gw = np.stack([full.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    assert np.array_equal(bits(gw), bits(ow))
+    full.close()
+
+
 # ------------------------------------------------------------------------------- API behaviour
 
 def test_custom_matching_and_unpaired(H, oracle_mod):
