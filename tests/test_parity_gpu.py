@@ -200,7 +200,8 @@ def test_uniform_sweep_points(H, oracle_mod):
 
 # ------------------------------------------------------------------------------- shared pair storage
 
-@pytest.mark.parametrize("S,G,bf16", [(2, 2, False), (4, 4, False), (16, 4, False), (8, 8, True), (6, 3, False), (1, 2, False)])
+@pytest.mark.parametrize("S,G,bf16", [(2, 2, False), (4, 4, False), (16, 4, False), (8, 8, True), (6, 3, False), (1, 2, False),
+                                      (8, 1, False), (8, 8, False), (6, 1, True)])
 @pytest.mark.parametrize("exact", [True, False])
 def test_share_pair_weights_equals_oracle(H, oracle_mod, S, G, bf16, exact):
     """HADPSGD_SHARE_PAIR_WEIGHTS: one weight buffer per pair, tile-major walk -- same arithmetic, so
