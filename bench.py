@@ -650,6 +650,15 @@ def run_ours(args):
                 "kernel": "hadpsgd::step_kernel (one launch = one step)", "frac_of_8TBps_nominal": achieved / 8000.0,
                 "note": "peak is a 1:1 copy; this kernel reads more than it writes, and reads are the faster direction, "
                         "so frac may exceed 1 (see ceiling)"}
+        if "nvlink_read_bytes_per_rank_per_step" in info:
+            # fused compute + peer-read kernel: the floor of a step is the slower of its local HBM bytes at the
+            # measured HBM peak and its NVLink bytes at the measured peer-copy rate (B200_PROFILING.md: 770 GB/s)
+            nv = info["nvlink_read_bytes_per_rank_per_step"]
+            floors = [max(abytes_rank / (peak * 1e9), b / 770e9) for b in nv]
+            roof["nvlink"] = {"read_bytes_per_rank": {"even_step": nv[0], "odd_step": nv[1]}, "peer_gbs_reference": 770.0,
+                              "floor_ms_even_odd": [f * 1e3 for f in floors],
+                              "frac_of_floor": (sum(floors) / len(floors)) / t_step,
+                              "note": "floor = max(local bytes / measured HBM peak, peer bytes / 770 GB/s) per step parity"}
         if not args.no_ceiling and world == 1:
             rd = S_rank * P_rank * (cfg["G"] * cfg["b_g"] + 8)
             ceil = mix_ceiling(torch, rd, abytes_rank - rd)
