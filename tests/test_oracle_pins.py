@@ -473,6 +473,29 @@ def test_zero_gradient_preserves_mean_and_contracts(oracle_mod, S):
     assert D_prev <= 1e-3 * oracle_mod.consensus_distance(rand((S, P), 20 + S, 0.05))
 
 
+def test_mixing_equal_columns_is_the_identity_down_to_subnormals(oracle_mod):
+    """T_k is doubly stochastic: mixing columns that are already equal changes nothing.
+    In fp32 that holds for EVERY finite value only in the stated order 0.5f * (a + a) -- a + a is exact
+    (also for subnormals), and halving it is exact again -- while 0.5f*a + 0.5f*a loses the last bit of
+    an odd subnormal.  No flush-to-zero (R17).  And where a + a overflows (|a| > FLT_MAX / 2) the stated
+    order gives Inf: IEEE propagation, not a rescue (R17)."""
+    tiny = np.float32(1e-45)                                   # the smallest subnormal
+    vals = np.array([tiny, -tiny, 3 * tiny, 5 * tiny, 1.1754942e-38, 1.1754944e-38, 0.0, -0.0, 1.0, -2.5e-7,
+                     1.7e38, -1.7e38], np.float32)
+    P = len(vals)
+    for S, k in ((2, 0), (4, 0), (4, 1), (8, 1)):
+        w = np.ascontiguousarray(np.tile(vals, (S, 1)))
+        v, g = np.zeros((S, P), np.float32), np.zeros((S, 2, P), np.float32)
+        with np.errstate(all="ignore"):
+            oracle_mod.step(g, w, v, LR, MU, k)
+        assert np.array_equal(bits(w), bits(np.tile(vals, (S, 1)))), (S, k)
+        assert not v.any()
+    w = np.full((2, 2), 3.0e38, np.float32)
+    with np.errstate(all="ignore"):
+        oracle_mod.step(np.zeros((2, 1, 2), np.float32), w, np.zeros((2, 2), np.float32), LR, MU, 0)
+    assert np.all(np.isposinf(w))                             # u_s + u_p overflows before the halving
+
+
 def test_consensus_exact_after_one_step_S2_two_steps_S4(oracle_mod):
     P = 300
     for S, steps in ((2, 1), (4, 2)):
