@@ -202,8 +202,14 @@ int hadpsgd_weights_bf16(hadpsgd_handle h, int s, void** dev_ptr);
 int hadpsgd_segment(hadpsgd_handle h, int seg, int64_t* elem_offset, int64_t* elem_len);
 int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded);
 
-/* Synchronises the stream and copies the diagnostics of the most recent step to the host. */
+/* Synchronises the stream and copies the diagnostics of the most recent step THAT COMPUTED THEM to the
+ * host (host_out->step_k says which).                                                               */
 int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out);
+/* Switch a5 off / on for the steps that follow (default: on, unless created with HADPSGD_NO_DIAG, which
+ * cannot be switched on).  A caller that looks at the diagnostics every N steps only pays for them
+ * there: for a small problem their final cross-block reduction is most of a step.
+ * Results (w, v) do not depend on it.  Host-only state: no stream work.                               */
+int hadpsgd_set_diagnostics(hadpsgd_handle h, int enable);
 
 /* Consensus distance D = sum_i sum_s (w_s[i] - mean_s w_.[i])^2 of the current weights
  * (mixing alone drives every learner to the mean; D measures how far they are).

@@ -85,6 +85,7 @@ def lib():
         L.hadpsgd_peer_flush.argtypes = [vp]
         L.hadpsgd_plan_peer.argtypes = [i32, i32, i32p, i32p, u64, i32p, i32p, i32p, i32p, i32p, i32p]
         L.hadpsgd_set_launch.argtypes = [vp, i32]
+        L.hadpsgd_set_diagnostics.argtypes = [vp, i32]
         L.hadpsgd_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.hadpsgd_error_string.argtypes = [i32]
         L.hadpsgd_error_string.restype = ctypes.c_char_p
@@ -309,6 +310,9 @@ class Hadpsgd:
 
     def hadpsgd_peer_flush(self):
         _check(lib().hadpsgd_peer_flush(self.h), self.h)
+
+    def hadpsgd_set_diagnostics(self, enable):
+        _check(lib().hadpsgd_set_diagnostics(self.h, 1 if enable else 0), self.h)
 
     def hadpsgd_set_launch(self, blocks_per_sm=0):
         _check(lib().hadpsgd_set_launch(self.h, blocks_per_sm), self.h)

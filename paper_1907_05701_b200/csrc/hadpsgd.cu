@@ -35,6 +35,8 @@ struct hadpsgd_ctx {
     int last_n_pairs = 0;
     uint64_t launches = 0;
     int blocks_per_sm = 0;   // tuning override of the persistent grid (0 = the plan's default)
+    bool diag_on = true;     // hadpsgd_set_diagnostics: a5 computed by the steps that follow (never with NO_DIAG)
+    uint64_t diag_step_k = 0;   // step_k of the most recent step that computed diagnostics
     std::vector<int32_t> partner;   // scratch of the step calls (no allocation per step)
     StepPlan plan;
     // super-learner partition (HADPSGD_PEER)
@@ -90,7 +92,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
                  int64_t elem_begin, int64_t elem_end, bool accumulate) {
     const bool bf16 = h->L.grad_dtype == HADPSGD_BF16;
     const bool exact = h->flags & HADPSGD_DETERMINISTIC;
-    const bool diag = !(h->flags & HADPSGD_NO_DIAG);
+    const bool diag = !(h->flags & HADPSGD_NO_DIAG) && h->diag_on;
     const bool emit = h->L.working_dtype == HADPSGD_BF16;
     const int wmode = (wmode_req == kSlots && mode != kPair) ? kOwn : wmode_req;
     LaunchPlan plan = emit ? (bf16 ? plan_bf16_emit(h->L.G, exact, diag, mode, wmode) : plan_f32_emit(h->L.G, exact, diag, mode, wmode))
@@ -191,7 +193,7 @@ int step_range(hadpsgd_ctx* h, const StepPlan& sp, float lr, float mu, int64_t e
     // buffers -- exactly the kOwn pair kernel -- and a single without one (unmixed, or publishing u for
     // a partner in another arena) is the ordinary kSingle kernel, which addresses weights through the
     // item's buffer indices anyway.  The plain kernels do not know pend_wsq / pend_gap: clear them.
-    if (!(h->flags & HADPSGD_NO_DIAG) && !accumulate)
+    if (!(h->flags & HADPSGD_NO_DIAG) && h->diag_on && !accumulate)
         CUDA_TRY(h, cudaMemsetAsync(h->d_diag + 3 * h->L.S, 0, sizeof(double) * 2 * h->L.S, h->stream));
     std::vector<WorkItem> part[2][2];   // [pairs | singles][plain | pending]
     for (const WorkItem& it : sp.pairs) part[0][(it.b_s || it.b_p) ? 1 : 0].push_back(it);
@@ -265,6 +267,7 @@ int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp, std::
 void commit_plan(hadpsgd_ctx* h, const StepPlan& sp, const std::vector<int32_t>& new_slot,
                  const std::vector<int32_t>& new_pending, uint64_t step_k) {
     h->last_step_k = step_k;
+    if (h->diag_on) h->diag_step_k = step_k;
     h->last_n_pairs = static_cast<int>(sp.pairs.size());
     if (is_peer(h)) { h->pending = new_pending; h->epoch++; }
     else h->w_slot = new_slot;
@@ -507,7 +510,7 @@ extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
     std::vector<double> tmp(kDiagArrays * S);
     CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * kDiagArrays * S, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    host_out->S = S; host_out->n_pairs = h->last_n_pairs; host_out->step_k = h->last_step_k;
+    host_out->S = S; host_out->n_pairs = h->last_n_pairs; host_out->step_k = h->diag_step_k;
     std::memcpy(host_out->gsq, tmp.data(), sizeof(double) * S);
     std::memcpy(host_out->wsq, tmp.data() + S, sizeof(double) * S);
     std::memcpy(host_out->gap, tmp.data() + 2 * S, sizeof(double) * S);
@@ -641,11 +644,18 @@ extern "C" int hadpsgd_peer_flush(hadpsgd_handle h) {
     const float* a_stage = reinterpret_cast<const float*>(h->arena + h->L.stage_off) + static_cast<size_t>(rd) * h->L.S * h->L.P_padded;
     launch_peer_flush(reinterpret_cast<float*>(h->arena + h->L.w_off), a_stage, h->d_peer, members.data(),
                       static_cast<int>(members.size() / 2), h->L.P_padded, h->L.S, h->num_sms,
-                      (h->flags & HADPSGD_NO_DIAG) ? nullptr : h->d_partials, h->d_diag,
+                      ((h->flags & HADPSGD_NO_DIAG) || !h->diag_on) ? nullptr : h->d_partials, h->d_diag,
                       (h->flags & HADPSGD_DETERMINISTIC) != 0, h->stream, &e);
     CUDA_TRY(h, e);
     h->launches++;
     h->pending.assign(h->L.S, -1);
+    return HADPSGD_OK;
+}
+
+extern "C" int hadpsgd_set_diagnostics(hadpsgd_handle h, int enable) {
+    if (!h) return HADPSGD_INVALID_ARG;
+    if (enable && (h->flags & HADPSGD_NO_DIAG)) { h->err = "handle was created with HADPSGD_NO_DIAG"; return HADPSGD_INVALID_ARG; }
+    h->diag_on = enable != 0;
     return HADPSGD_OK;
 }
 

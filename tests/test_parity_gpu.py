@@ -170,7 +170,7 @@ def test_odd_S_without_mixing(H, oracle_mod):
 
 
 def test_max_S(H, oracle_mod):
-    """S = HADPSGD_MAX_S = 512 super-learners (256 pairs in the kernel's work table)."""
+    """S = HADPSGD_MAX_S = 512 super-learners (256 pairs: eight launches of 32 work items)."""
     gw, gv, ow, ov = run_both(H, oracle_mod, 512, 1, [2_000], 2, flags=H.DETERMINISTIC, seed=51)
     assert_parity(gw, gv, ow, ov, True)
 
@@ -615,7 +615,7 @@ def test_matching_sequences_with_diagnostics(H, oracle_mod, flagname, bf16, exac
 
 
 def test_max_S_unmixed_diagnostics_span_several_launches(H, oracle_mod):
-    """S = 512 unmixed super-learners = 512 single items > kMaxWork: several launches feed one
+    """S = 512 unmixed super-learners = 512 single items, 32 per launch: sixteen launches feed one
     diagnostics record (gap exactly 0 everywhere)."""
     gw, gv, ow, ov = run_both(H, oracle_mod, 512, 2, [3_001], 2, flags=H.DETERMINISTIC | H.NO_MIX, seed=52)
     assert_parity(gw, gv, ow, ov, True)
@@ -764,6 +764,36 @@ def test_library_owned_arena_and_two_streams(H, oracle_mod, torch_cuda):
         gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
         assert_parity(gw, gv, ow, ov, True)
         h.close()
+
+
+def test_diagnostics_can_be_switched_off_for_some_steps(H, oracle_mod):
+    """hadpsgd_set_diagnostics: steps without a5 give the same w, v; hadpsgd_diagnostics() keeps returning
+    the record of the last step that computed them."""
+    from fixtures import problem
+    S, G, P, seed = 4, 2, 50_021, 191
+    h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC)
+    problem.fill_weights(h, seed)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    kept = None
+    for k in range(6):
+        h.hadpsgd_set_diagnostics(k % 3 == 0)                       # steps 0 and 3 only
+        problem.fill_grads(h, seed, k)
+        h.hadpsgd_step(LR, MU, k)
+        od = oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k, diag=True)
+        gd = h.hadpsgd_diagnostics()
+        if k % 3 == 0:
+            kept = od
+        assert gd["step_k"] == (k // 3) * 3
+        assert_diag(gd, kept, k)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    assert_parity(gw, gv, ow, ov, True)
+    h.close()
+    nd = H.Hadpsgd(2, 2, [100], H.F32, H.NO_DIAG)
+    with pytest.raises(H.HadpsgdError):
+        nd.hadpsgd_set_diagnostics(True)
+    nd.hadpsgd_set_diagnostics(False)
+    nd.close()
 
 
 def test_diagnostics_are_run_to_run_deterministic(H):
