@@ -52,12 +52,15 @@ int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
     L.g_off = cur; cur = round_up(cur + static_cast<size_t>(S) * G * L.g_stride_bytes(), kRegionAlign);
     L.wb_off = cur;
     if (L.working_dtype == HADPSGD_BF16) cur = round_up(cur + static_cast<size_t>(S) * L.P_padded * 2, kRegionAlign);
-    // aux: per-block partial sums [kMaxGridBlocks][items per launch x quantities] doubles, the results
-    // (kDiagArrays x S doubles), the ticket
+    // aux: per-block partial sums of the step kernel [kMaxGridBlocks][items per launch x quantities], 16 B
+    // each (a double with its launch tag, step_kernel.cuh); a plain scratch of doubles for the consensus
+    // and flush kernels; the results (kDiagArrays x S doubles)
     const int items = S < kMaxItemsPerLaunch ? S : kMaxItemsPerLaunch;
     L.aux_off = cur;
-    L.aux_bytes = round_up(static_cast<size_t>(items) * kMaxDiagQuantities * kMaxGridBlocks * sizeof(double) +
-                           static_cast<size_t>(kDiagArrays * S) * sizeof(double) + 256, kRegionAlign);
+    L.partials_bytes = round_up(static_cast<size_t>(items) * kMaxDiagQuantities * kMaxGridBlocks * 16, kRegionAlign);
+    L.scratch_bytes = round_up(static_cast<size_t>(kMaxGridBlocks) * kMaxItemsPerLaunch * 2 * sizeof(double), kRegionAlign);
+    L.aux_bytes = L.partials_bytes + L.scratch_bytes +
+                  round_up(static_cast<size_t>(kDiagArrays * S) * sizeof(double) + 256, kRegionAlign);
     cur += L.aux_bytes;
     L.total_bytes = cur;
     *out = L;

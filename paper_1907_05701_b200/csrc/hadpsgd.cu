@@ -28,9 +28,10 @@ struct hadpsgd_ctx {
     std::vector<int32_t> w_slot;                           // slot (buffer index) that holds w_s right now
     char* arena = nullptr;
     bool owns_arena = false;
-    double* d_partials = nullptr;
+    TaggedDouble* d_partials = nullptr;   // step kernel: block partials with their launch tag
+    double* d_scratch = nullptr;           // consensus / flush kernels: block partials, plain doubles
     double* d_diag = nullptr;
-    unsigned int* d_ticket = nullptr;
+    uint32_t diag_tag = 0;                 // tag of the block partials of the most recent launch (never 0)
     uint64_t last_step_k = 0;
     int last_n_pairs = 0;
     uint64_t launches = 0;
@@ -115,7 +116,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     a.invG = 1.0f / static_cast<float>(h->L.G);   // fp32 reciprocal, exact for G = 1,2,4,8 (R5)
     a.accumulate_diag = accumulate ? 1 : 0;
     a.S = h->L.S;
-    a.partials = h->d_partials; a.diag = h->d_diag; a.ticket = h->d_ticket;
+    a.partials = h->d_partials; a.diag = h->d_diag; a.tag = ++h->diag_tag ? h->diag_tag : ++h->diag_tag;
     for (int j = 0; j < n_items; ++j) {
         const WorkItem& it = items[j];
         a.items[j] = {static_cast<unsigned short>(it.s), static_cast<unsigned short>(it.p),
@@ -124,15 +125,9 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
                       static_cast<unsigned short>(it.b_s), static_cast<unsigned short>(it.b_p)};
     }
 
-    // per-warp diagnostic accumulators [warps][items][quantities]; the last block's column sums reuse
-    // the buffer and need max(threads, rows) doubles.  At most 18 KB: no opt-in needed.
+    // per-warp diagnostic accumulators [warps][items][quantities].  At most 18 KB: no opt-in needed.
     const int nq = plan.wmode == kPeer ? kNQPeer : kNQ;
-    size_t smem = 0;
-    if (diag) {
-        size_t cells = static_cast<size_t>(plan.threads / 32) * n_items * nq;
-        if (cells < static_cast<size_t>(plan.threads)) cells = plan.threads;
-        smem = cells * sizeof(double);
-    }
+    const size_t smem = diag ? static_cast<size_t>(plan.threads / 32) * n_items * nq * sizeof(double) : 0;
     int occ = 0;
     for (const auto& kv : h->occupancy) if (kv.first == plan.fn) occ = kv.second;
     if (occ == 0) {   // with the largest shared-memory footprint this kernel can be launched with
@@ -151,7 +146,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     if (grid > want) grid = want;
     if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;
     if (grid < 1) grid = 1;
-    // how many blocks work on any one item (the last block sums exactly their partials)
+    // how many blocks work on any one item (the collecting block sums exactly their partials)
     long long per = grid;
     if (plan.wmode == kSlots) {                      // tile-major walk: blocks (i * n_work + j) mod grid
         long long x = a.n_work, y = grid;
@@ -362,10 +357,9 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
         delete h; return HADPSGD_CUDA;
     }
     char* aux = h->arena + L.aux_off;
-    const int items = S < kMaxItemsPerLaunch ? S : kMaxItemsPerLaunch;
-    h->d_partials = reinterpret_cast<double*>(aux);
-    h->d_diag = h->d_partials + static_cast<size_t>(items) * kMaxDiagQuantities * kMaxGridBlocks;
-    h->d_ticket = reinterpret_cast<unsigned int*>(h->d_diag + kDiagArrays * S);
+    h->d_partials = reinterpret_cast<TaggedDouble*>(aux);
+    h->d_scratch = reinterpret_cast<double*>(aux + L.partials_bytes);
+    h->d_diag = reinterpret_cast<double*>(aux + L.partials_bytes + L.scratch_bytes);
     *out = h;
     return HADPSGD_OK;
 }
@@ -535,14 +529,14 @@ extern "C" int hadpsgd_consensus(hadpsgd_handle h, double* D_out) {
     if (!h || !D_out) return HADPSGD_INVALID_ARG;
     if (is_peer(h)) { h->err = "hadpsgd_consensus needs all S_global weight columns in one arena: not on a HADPSGD_PEER handle"; return HADPSGD_INVALID_ARG; }
     DeviceGuard guard(h->device);
-    // the partials scratch is free between steps: everything is ordered on h->stream
+    // the scratch is free between steps: everything is ordered on h->stream
     cudaError_t e = cudaSuccess;
     const int grid = launch_consensus(reinterpret_cast<const float*>(h->arena + h->L.w_off), h->L.P_padded, h->L.S,
-                                      h->w_slot.data(), h->num_sms, h->d_partials, h->stream, &e);
+                                      h->w_slot.data(), h->num_sms, h->d_scratch, h->stream, &e);
     CUDA_TRY(h, e);
     h->launches++;
     std::vector<double> part(grid);
-    CUDA_TRY(h, cudaMemcpyAsync(part.data(), h->d_partials, sizeof(double) * grid, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(part.data(), h->d_scratch, sizeof(double) * grid, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     double D = 0.;
     for (int b = 0; b < grid; ++b) D += part[b];   // fixed order: run-to-run deterministic
@@ -644,7 +638,7 @@ extern "C" int hadpsgd_peer_flush(hadpsgd_handle h) {
     const float* a_stage = reinterpret_cast<const float*>(h->arena + h->L.stage_off) + static_cast<size_t>(rd) * h->L.S * h->L.P_padded;
     launch_peer_flush(reinterpret_cast<float*>(h->arena + h->L.w_off), a_stage, h->d_peer, members.data(),
                       static_cast<int>(members.size() / 2), h->L.P_padded, h->L.S, h->num_sms,
-                      ((h->flags & HADPSGD_NO_DIAG) || !h->diag_on) ? nullptr : h->d_partials, h->d_diag,
+                      ((h->flags & HADPSGD_NO_DIAG) || !h->diag_on) ? nullptr : h->d_scratch, h->d_diag,
                       (h->flags & HADPSGD_DETERMINISTIC) != 0, h->stream, &e);
     CUDA_TRY(h, e);
     h->launches++;

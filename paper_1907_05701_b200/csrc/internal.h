@@ -24,7 +24,8 @@ struct Layout {
     size_t w_off = 0, v_off = 0, g_off = 0;  // byte offsets inside the arena
     size_t stage_off = 0;                    // = w_off + S weight buffers: [2][S] stage buffers (peer_stage only)
     size_t wb_off = 0;                       // bf16 working copies (S x P_padded x 2 B), if any
-    size_t aux_off = 0, aux_bytes = 0;       // diagnostics scratch (partials, results, ticket)
+    size_t aux_off = 0, aux_bytes = 0;       // diagnostics scratch: tagged partials | plain scratch | results
+    size_t partials_bytes = 0, scratch_bytes = 0;
     size_t total_bytes = 0;
     size_t grad_elem_bytes() const { return grad_dtype == HADPSGD_BF16 ? 2 : 4; }
     size_t w_stride_bytes() const { return static_cast<size_t>(P_padded) * 4; }

@@ -24,8 +24,8 @@
 //
 // Diagnostics: per tile, per-thread sums -> warp shuffle tree -> the warp's own accumulator of
 // that work item in shared memory (no atomics, no block barrier per tile) -> at the end one block
-// partial per item in a fixed slot of global scratch -> the last block to finish (ticket) reduces
-// the partials in a fixed order.  Results are therefore run-to-run deterministic.  A launch of a
+// partial per item in a fixed slot of global scratch, tagged with the launch's number -> the last
+// block of the grid polls the tags and adds the partials in a fixed order (no fence, no atomics).  Results are therefore run-to-run deterministic.  A launch of a
 // single block skips the scratch round trip and reduces straight from shared memory.
 #pragma once
 #include <cuda_bf16.h>
@@ -52,6 +52,14 @@ enum WMode : int { kOwn = 0, kSlots = 1, kPeer = 2, kChain = 3 };
 // -- the 2S stage buffers).
 struct Item { unsigned short s, p, a_s, a_p, o_s, o_p, b_s, b_p; };
 
+// A block partial on its way to the collecting block: lo = (tag << 32) | low half of the double,
+// hi = (tag << 32) | high half.  Each word is one 64-bit access, so a reader that finds the tag of
+// THIS launch in both words holds the value -- the flag travels with the data and no fence is needed.
+// A tag is never 0, the scratch is zero at create, and the reader zeroes every slot it has consumed,
+// so between launches the scratch is all zero: a launch replayed with the same tag (a CUDA graph) is
+// safe, and the host still changes the tag with every launch it enqueues.
+struct __align__(16) TaggedDouble { unsigned long long lo, hi; };
+
 struct StepArgs {
     float* w;             // weight buffers (main, then stage) of P floats each
     float* v;             // S buffers of P floats
@@ -61,9 +69,9 @@ struct StepArgs {
     long long P;          // padded elements per buffer
     long long unit_begin; // first vector unit of this launch
     long long unit_end;   // one past the last vector unit
-    double* partials;     // [gridDim.x][n_work * NQ]
+    TaggedDouble* partials;   // [gridDim.x][n_work * NQ]
     double* diag;         // gsq[S] | wsq[S] | gap[S] | pend_wsq[S] | pend_gap[S]
-    unsigned int* ticket;
+    unsigned int tag;     // never 0; the host changes it with every launch it enqueues
     int G;
     int n_work;
     int S;
@@ -266,6 +274,32 @@ __device__ __forceinline__ void resolve_pending(Vec<UNIT>& w, const Vec<UNIT>& b
     if constexpr (DIAG) { d_wsq += static_cast<double>(sw); d_gap += static_cast<double>(sg); }
 }
 
+__device__ __forceinline__ void st_tagged(TaggedDouble* p, double x, unsigned tag) {
+    const unsigned long long b = static_cast<unsigned long long>(__double_as_longlong(x));
+    const unsigned long long t = static_cast<unsigned long long>(tag) << 32;
+    asm volatile("st.volatile.global.v2.u64 [%0], {%1,%2};" :: "l"(p), "l"(t | (b & 0xffffffffull)), "l"(t | (b >> 32)) : "memory");
+}
+__device__ __forceinline__ TaggedDouble ld_tagged(const TaggedDouble* p) {
+    TaggedDouble r;
+    asm volatile("ld.volatile.global.v2.u64 {%0,%1}, [%2];" : "=l"(r.lo), "=l"(r.hi) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void clear_tagged(TaggedDouble* p) {
+    asm volatile("st.volatile.global.v2.u64 [%0], {%1,%1};" :: "l"(p), "l"(0ull) : "memory");
+}
+// Value of a partial already loaded once (t); re-polls until both words carry `tag`.  The writer is a
+// block of the same grid that is resident or finished, so the wait is short; a bounded spin turns
+// a protocol error into NaN diagnostics instead of a hung GPU.
+__device__ __forceinline__ double wait_tagged(const TaggedDouble* p, TaggedDouble t, unsigned tag) {
+    unsigned spins = 0;
+    while (static_cast<unsigned>(t.lo >> 32) != tag || static_cast<unsigned>(t.hi >> 32) != tag) {
+        if (++spins > (1u << 26)) return __longlong_as_double(0x7ff8000000000000ll);   // about a minute
+        if (spins > 16) __nanosleep(spins > 4096 ? 512 : 32);
+        t = ld_tagged(p);
+    }
+    return __longlong_as_double(static_cast<long long>((t.hi << 32) | (t.lo & 0xffffffffull)));
+}
+
 __device__ __forceinline__ double warp_sum(double x) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
@@ -299,7 +333,6 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     constexpr int WARPS = THREADS / 32;
     constexpr int NQ = PEER ? kNQPeer : kNQ;
     extern __shared__ double s_acc[];    // DIAG: [WARPS][n_work][NQ], each warp owns its rows
-    __shared__ unsigned int s_last;
 
     const int tid = threadIdx.x;
     const long long n_units = a.unit_end - a.unit_begin;
@@ -572,60 +605,58 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             }
             return;
         }
-        // block partial of the rows of every item this block worked on -> partials[block][row]
+        // Block partial of the rows of every item this block worked on -> partials[block][row], TAGGED:
+        // the two halves of the double travel in two 64-bit words whose upper halves carry this launch's
+        // tag, so a reader that sees both tags has the value -- no fence, no ticket, no atomics, and no
+        // block waits for its data stores to drain.
         for (int row = tid; row < R; row += THREADS) {
             if (!((touched >> (row / NQ)) & 1u)) continue;
             double tot = 0.;
             for (int wi = 0; wi < WARPS; ++wi) tot += s_acc[static_cast<size_t>(wi) * R + row];       // fixed order
-            a.partials[static_cast<size_t>(blockIdx.x) * R + row] = tot;
+            st_tagged(a.partials + static_cast<size_t>(blockIdx.x) * R + row, tot, a.tag);
         }
-        // The last block to arrive reduces all block partials in a fixed order.  Order matters: every
-        // thread's partial stores, then its fence, then a block barrier, and only then the ticket --
-        // otherwise warp 0 could publish the ticket before another warp's partials are out.
-        __threadfence();
-        __syncthreads();
-        if (tid == 0) {
-            unsigned int t = atomicAdd(a.ticket, 1u);
-            s_last = (t == gridDim.x - 1) ? 1u : 0u;
-        }
-        __syncthreads();
-        if (!s_last) return;
-        __threadfence();
-        // Item j was worked on by exactly touch_count blocks: the i-th of them (in tile order) is block
-        // (j * n_tiles + i) mod grid in the item-major walk; in the CHAIN walk it is every block.  Only their partials are read (for a small problem that is one block per tile instead of
-        // the whole grid), with every thread busy: thread (c, row) sums contributors c, c+C, c+2C, ... of
-        // its row (independent loads), then the C column sums of a row are added in order.  The result
-        // depends on the launch shape only: run-to-run deterministic.
-        const int C = (THREADS / R) > 0 ? (THREADS / R) : 1;
-        double* s_col = s_acc;           // reuse: C x R <= max(THREADS, R) doubles (the host sizes it)
+        // Item j is COLLECTED by block grid-1 - (j mod grid): the blocks with the highest ids, which are
+        // dispatched last and have the fewest tiles.  Every other block is done here.  (The whole grid is
+        // resident at once -- the host sizes it so -- hence a collector never waits for a block that
+        // cannot run.)  Item j was worked on by exactly touch_count blocks: the i-th of them (in tile
+        // order) is block (j * n_tiles + i) mod grid in the item-major walk, (j + i * n_work) mod grid in the
+        // tile-major walk, block i in the CHAIN walk.  One warp per quantity: lane l polls contributors l,
+        // l+32, ... (eight independent loads at a time), adds them in that order, the lanes combine in a
+        // fixed shuffle tree, and each consumed slot is zeroed again for the launches that follow.  The
+        // result depends on the launch shape only: run-to-run deterministic.
         const unsigned nb = gridDim.x;
-        // contributor i of item j is block (first + i * step1) mod nb; walked incrementally (no division
-        // inside the loop).  Item-major: first = j * n_tiles, step 1.  Tile-major: first = j, step n_work.
-        // CHAIN: every block works on every item.
-        const unsigned step1 = TILE_MAJOR ? static_cast<unsigned>(a.n_work) % nb : 1u % nb;
-        const unsigned stepC = static_cast<unsigned>((static_cast<unsigned long long>(step1) * C) % nb);
-        for (int task = tid; task < R * C; task += THREADS) {
-            const int c = task / R, row = task - c * R;
-            const unsigned j = row / NQ;
+        const int lane = tid & 31, warp = tid >> 5;
+        for (int j = static_cast<int>(nb - 1u - blockIdx.x); j < a.n_work; j += static_cast<int>(nb)) {
             const unsigned long long first = CHAIN ? 0ull : TILE_MAJOR ? static_cast<unsigned long long>(j)
                                                    : static_cast<unsigned long long>(j) * static_cast<unsigned long long>(n_tiles);
-            unsigned b = static_cast<unsigned>((first + static_cast<unsigned long long>(step1) * c) % nb);
-            double sum = 0.;
-#pragma unroll 4
-            for (int i = c; i < a.touch_count; i += C) {
-                sum += __ldcg(a.partials + static_cast<size_t>(b) * R + row);
-                b += stepC;
-                if (b >= nb) b -= nb;
+            const unsigned long long step1 = TILE_MAJOR ? static_cast<unsigned long long>(a.n_work) : 1ull;
+            for (int k = warp; k < NQ; k += WARPS) {
+                const int row = j * NQ + k;
+                double sum = 0.;
+                for (int i0 = lane; i0 < a.touch_count; i0 += 32 * 8) {
+                    TaggedDouble* src[8];
+                    TaggedDouble t[8];
+#pragma unroll
+                    for (int m = 0; m < 8; ++m) {
+                        const int i = i0 + 32 * m;
+                        if (i < a.touch_count) {
+                            const unsigned b = static_cast<unsigned>((first + step1 * static_cast<unsigned long long>(i)) % nb);
+                            src[m] = a.partials + static_cast<size_t>(b) * R + row;
+                            t[m] = ld_tagged(src[m]);
+                        }
+                    }
+#pragma unroll
+                    for (int m = 0; m < 8; ++m) {
+                        if (i0 + 32 * m < a.touch_count) {
+                            sum += wait_tagged(src[m], t[m], a.tag);
+                            clear_tagged(src[m]);
+                        }
+                    }
+                }
+                sum = warp_sum(sum);
+                if (lane == 0) publish(row, sum);
             }
-            s_col[task] = sum;
         }
-        __syncthreads();
-        for (int row = tid; row < R; row += THREADS) {
-            double sum = 0.;
-            for (int c = 0; c < C; ++c) sum += s_col[c * R + row];
-            publish(row, sum);
-        }
-        if (tid == 0) *a.ticket = 0u;  // re-arm for the next launch on this stream
     }
 }
 
