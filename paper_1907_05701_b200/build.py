@@ -20,7 +20,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
+    extra = os.environ.get("HADPSGD_NVCC_EXTRA", "").split()     # development: extra -D switches
+    cmd = [nvcc, *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
            *[os.path.join(CSRC, s) for s in SOURCES]]
     subprocess.run(cmd, check=True, cwd=HERE)
     return LIB

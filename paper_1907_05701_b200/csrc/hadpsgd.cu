@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <utility>
@@ -31,6 +32,10 @@ struct hadpsgd_ctx {
     TaggedDouble* d_partials = nullptr;   // step kernel: block partials with their launch tag
     double* d_scratch = nullptr;           // consensus / flush kernels: block partials, plain doubles
     double* d_diag = nullptr;
+    bool walk_reverse = false;             // direction of the kernel's walk; flips with every step (L2 reuse)
+    bool serpentine = true;
+    size_t keep_bytes = size_t(64) << 20;  // bytes stored at the end of a step's walk that stay in L2
+    bool use_pdl = true;                   // launch steps with programmatic stream serialization
     uint32_t diag_tag = 0;                 // tag of the block partials of the most recent launch (never 0)
     uint64_t last_step_k = 0;
     int last_n_pairs = 0;
@@ -74,6 +79,8 @@ int launch_peer_flush(float* w_main, const float* a_stage, const float* const* p
 // ---- kernel dispatch -------------------------------------------------------------------
 namespace {
 
+constexpr size_t kKeepMaxStepBytes = size_t(2) << 30;
+
 // Entry points that enqueue work make the handle's device current for their duration, so a
 // process that drives several GPUs may call them from any current device.
 struct DeviceGuard {
@@ -115,6 +122,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     a.lr = lr; a.mu = mu;
     a.invG = 1.0f / static_cast<float>(h->L.G);   // fp32 reciprocal, exact for G = 1,2,4,8 (R5)
     a.accumulate_diag = accumulate ? 1 : 0;
+    a.reverse = h->walk_reverse ? 1 : 0;
     a.S = h->L.S;
     a.partials = h->d_partials; a.diag = h->d_diag; a.tag = ++h->diag_tag ? h->diag_tag : ++h->diag_tag;
     for (int j = 0; j < n_items; ++j) {
@@ -143,6 +151,10 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     // shared slots: a block owns whole tiles (and walks every item of each); else (item, tile) pairs
     long long want = plan.wmode == kChain ? n_tiles : n_tiles * a.n_work;
     long long grid = static_cast<long long>(h->num_sms) * bps;
+    // a problem that fits ONE wave of resident blocks runs as one wave (every block exactly one tile,
+    // all tiles in flight at once) instead of some blocks walking two tiles one after the other:
+    // 2^18 parameters x 4 x 4 fp32 takes 5.9 instead of 7.2 us per step
+    if (h->blocks_per_sm == 0 && want <= static_cast<long long>(h->num_sms) * occ) grid = want;
     if (grid > want) grid = want;
     if (grid > kMaxGridBlocks) grid = kMaxGridBlocks;
     if (grid < 1) grid = 1;
@@ -153,9 +165,37 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
         while (y) { const long long t = x % y; x = y; y = t; }   // x = gcd(n_work, grid)
         per = grid / x;
     }
+    // Stores of the last part of the walk keep the default L2 policy -- the next step, walking the other
+    // way, begins with them -- everything before is evict_first.  The budget is in bytes STORED (a share
+    // of the 126 MB L2; where all of w and v fit they never travel to HBM at all); a step that moves
+    // more than kKeepMaxStepBytes gains nothing and loses 2-4 % (the kept lines shrink the L2 left for
+    // streaming), so it keeps nothing.
+    {
+        const long long walk_len = plan.wmode == kChain ? n_tiles : n_tiles * a.n_work;
+        const size_t members = mode == kSingle ? 1 : 2;
+        const size_t per_walk_pos = static_cast<size_t>(plan.tile_units) * 32 * members * (plan.wmode == kChain ? a.n_work : 1);
+        const size_t store_bytes = per_walk_pos * (bf16 ? 4 : 2) + (emit ? per_walk_pos * (bf16 ? 2 : 1) / 2 : 0);   // w, v (+ the bf16 copy of w)
+        const size_t all_bytes = per_walk_pos * (h->L.G + (bf16 ? 8 : 4));
+        long long keep_tiles = 0;
+        if (h->serpentine && all_bytes * static_cast<size_t>(walk_len) < kKeepMaxStepBytes)
+            keep_tiles = static_cast<long long>(h->keep_bytes / (store_bytes ? store_bytes : 1));
+        if (keep_tiles > walk_len) keep_tiles = walk_len;
+        a.keep_from = walk_len - keep_tiles;
+    }
     a.touch_count = static_cast<int>(plan.wmode == kChain ? grid : (n_tiles < per ? n_tiles : per));
     void* params[] = {&a};
-    CUDA_TRY(h, cudaLaunchKernel(plan.fn, dim3(static_cast<unsigned>(grid)), dim3(plan.threads), params, smem, h->stream));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(grid));
+    cfg.blockDim = dim3(plan.threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = h->stream;
+    // programmatic dependent launch: the kernel itself waits (griddepcontrol.wait) for the launch before it
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = h->use_pdl ? 1 : 0;
+    CUDA_TRY(h, cudaLaunchKernelExC(&cfg, plan.fn, params));
     h->launches++;
     return HADPSGD_OK;
 }
@@ -262,6 +302,7 @@ int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp, std::
 void commit_plan(hadpsgd_ctx* h, const StepPlan& sp, const std::vector<int32_t>& new_slot,
                  const std::vector<int32_t>& new_pending, uint64_t step_k) {
     h->last_step_k = step_k;
+    if (h->serpentine) h->walk_reverse = !h->walk_reverse;
     if (h->diag_on) h->diag_step_k = step_k;
     h->last_n_pairs = static_cast<int>(sp.pairs.size());
     if (is_peer(h)) { h->pending = new_pending; h->epoch++; }
@@ -333,6 +374,9 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
         if (!dt.peer_stage) { g_create_error = "HADPSGD_PEER needs dtypes.peer_stage = 1 (the stage buffers)"; return HADPSGD_INVALID_ARG; }
     }
     hadpsgd_ctx* h = new hadpsgd_ctx();
+    if (const char* e_pdl = std::getenv("HADPSGD_PDL")) h->use_pdl = e_pdl[0] != '0';   // development switch
+    if (const char* e_sp = std::getenv("HADPSGD_SERPENTINE")) h->serpentine = e_sp[0] != '0';   // development switch
+    if (const char* e_kb = std::getenv("HADPSGD_KEEP_MB")) h->keep_bytes = static_cast<size_t>(std::atoll(e_kb)) << 20;   // development switch
     h->w_slot.resize(S);
     for (int s = 0; s < S; ++s) h->w_slot[s] = s;
     h->pending.assign(S, -1);

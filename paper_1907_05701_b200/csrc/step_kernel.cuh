@@ -77,6 +77,8 @@ struct StepArgs {
     int S;
     int accumulate_diag;  // 0: diag = result ; 1: diag += result (chunked host path)
     int touch_count;      // blocks that work on any one item (host: from n_tiles, grid, walk order)
+    int reverse;          // 1: walk the (item, tile) space backwards
+    long long keep_from;  // walk position ((item, tile) index; CHAIN: tile index) from which stores stay in L2
     float lr, mu, invG;
     Item items[kInlineItems];
 };
@@ -88,18 +90,34 @@ struct StepArgs {
 // because fewer, longer DRAM bursts are in flight per stream.  (Selecting
 // the policy at run time -- evict_normal when one step's working set fits L2 -- measured no
 // faster at any L2-resident size and 0.4 % slower at full size, so the hint is a literal.)
+#ifndef HADPSGD_LD_L2
+#define HADPSGD_LD_L2 ".L2::evict_first"
+#endif
+#ifndef HADPSGD_ST_L2
+#define HADPSGD_ST_L2 ".L2::evict_first"
+#endif
 struct Raw8 { unsigned u[8]; };
 __device__ __forceinline__ Raw8 ld_stream32(const void* p) {
     Raw8 r;
-    asm volatile("ld.global.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+    asm volatile("ld.global.L1::no_allocate" HADPSGD_LD_L2 ".v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                  : "=r"(r.u[0]), "=r"(r.u[1]), "=r"(r.u[2]), "=r"(r.u[3]), "=r"(r.u[4]), "=r"(r.u[5]), "=r"(r.u[6]), "=r"(r.u[7])
                  : "l"(p));
     return r;
 }
-__device__ __forceinline__ void st_stream32(void* p, const Raw8& r) {
-    asm volatile("st.global.L1::no_allocate.L2::evict_first.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-                 :: "l"(p), "r"(r.u[0]), "r"(r.u[1]), "r"(r.u[2]), "r"(r.u[3]), "r"(r.u[4]), "r"(r.u[5]), "r"(r.u[6]), "r"(r.u[7])
-                 : "memory");
+// keep == false: L2::evict_first -- the line is written back and dropped as soon as possible (a step
+// of a large problem never sees it again before it would have been evicted anyway; measured 6 %
+// faster than evict_normal at >= 2 GB per step).  keep == true (block-uniform): the line stays in L2
+// like any other -- used for the last part of a step's walk, which the NEXT step, walking in the
+// opposite direction, reads and overwrites first (10-15 % at 0.2-0.8 GB per step).
+__device__ __forceinline__ void st_stream32(void* p, const Raw8& r, bool keep) {
+    if (keep)
+        asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                     :: "l"(p), "r"(r.u[0]), "r"(r.u[1]), "r"(r.u[2]), "r"(r.u[3]), "r"(r.u[4]), "r"(r.u[5]), "r"(r.u[6]), "r"(r.u[7])
+                     : "memory");
+    else
+        asm volatile("st.global.L1::no_allocate" HADPSGD_ST_L2 ".v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                     :: "l"(p), "r"(r.u[0]), "r"(r.u[1]), "r"(r.u[2]), "r"(r.u[3]), "r"(r.u[4]), "r"(r.u[5]), "r"(r.u[6]), "r"(r.u[7])
+                     : "memory");
 }
 
 template <bool EXACT> __device__ __forceinline__ float add_(float a, float b) { return EXACT ? __fadd_rn(a, b) : a + b; }
@@ -151,13 +169,13 @@ __device__ __forceinline__ void load_state(const float* base, long long off, Vec
     }
 }
 template <int UNIT>
-__device__ __forceinline__ void store_state(float* base, long long off, const Vec<UNIT>& in) {
+__device__ __forceinline__ void store_state(float* base, long long off, const Vec<UNIT>& in, bool keep) {
 #pragma unroll
     for (int q = 0; q < UNIT / 8; ++q) {
         Raw8 t;
 #pragma unroll
         for (int e = 0; e < 8; ++e) t.u[e] = __float_as_uint(in.x[8 * q + e]);
-        st_stream32(base + off + 8 * q, t);
+        st_stream32(base + off + 8 * q, t, keep);
     }
 }
 
@@ -168,7 +186,7 @@ __device__ __forceinline__ void store_state(float* base, long long off, const Ve
 // multiples of 64 elements -- so an even lane's unit and the next are live or dead together).
 // Must be called by all 32 lanes of the warp; `live` predicates the store only.
 template <int UNIT>
-__device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<UNIT>& in, bool live) {
+__device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<UNIT>& in, bool live, bool keep) {
     unsigned pk[UNIT / 2];
 #pragma unroll
     for (int q = 0; q < UNIT / 2; ++q) {
@@ -180,14 +198,14 @@ __device__ __forceinline__ void store_bf16(void* base, long long off, const Vec<
     if constexpr (UNIT == 16) {
 #pragma unroll
         for (int q = 0; q < 8; ++q) r.u[q] = pk[q];
-        if (live) st_stream32(dst, r);
+        if (live) st_stream32(dst, r, keep);
     } else {
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             r.u[q] = pk[q];
             r.u[4 + q] = __shfl_down_sync(0xffffffffu, pk[q], 1);
         }
-        if (live && (threadIdx.x & 1) == 0) st_stream32(dst, r);
+        if (live && (threadIdx.x & 1) == 0) st_stream32(dst, r, keep);
     }
 }
 
@@ -345,6 +363,14 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
         for (int idx = tid; idx < WARPS * a.n_work * NQ; idx += THREADS) s_acc[idx] = 0.;
         __syncthreads();
     }
+    // Programmatic dependent launch: the host launches every step with "programmatic stream
+    // serialization", so this grid may become resident while the launch before it on the stream is
+    // still draining.  Nothing above touches global memory; everything below waits here until that
+    // launch has completed and its writes are visible.  Then the NEXT launch is allowed in at once: its
+    // blocks park at this same line (one more resident block per SM fits beside a working one), so
+    // that back-to-back steps pay no launch latency between them.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     // Flattened (work item, tile) space; block b takes global tiles b, b+grid, ...
     //  item-major: tiles of item 0, then item 1, ...: for large P the whole chip streams one pair
@@ -399,15 +425,22 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
     for (long long gt = blockIdx.x; ; gt += gridDim.x, ++seq) {
         int j;
         long long tile;
+        bool keep;        // this tile lies in the last part of the walk: its stores stay in L2 (st_stream32)
+        // a.reverse: the same walk from its far end (the host alternates the direction from step to step,
+        // so a step begins with what the step before it touched last and may still find it in L2)
         if constexpr (CHAIN) {
             const long long round = seq / a.n_work;
             j = static_cast<int>(seq - round * a.n_work);
             tile = blockIdx.x + round * gridDim.x;
             if (tile >= n_tiles) break;
+            keep = tile >= a.keep_from;
+            if (a.reverse) tile = n_tiles - 1 - tile;
         } else {
             if (gt >= total_tiles) break;
-            if constexpr (TILE_MAJOR) { tile = gt / a.n_work; j = static_cast<int>(gt - tile * a.n_work); }
-            else { j = static_cast<int>(gt / n_tiles); tile = gt - static_cast<long long>(j) * n_tiles; }
+            keep = gt >= a.keep_from;
+            const long long g2 = a.reverse ? total_tiles - 1 - gt : gt;
+            if constexpr (TILE_MAJOR) { tile = g2 / a.n_work; j = static_cast<int>(g2 - tile * a.n_work); }
+            else { j = static_cast<int>(g2 / n_tiles); tile = g2 - static_cast<long long>(j) * n_tiles; }
         }
         const long long base = tile * TILE;
         bool take_carry = false, take_first = false;     // CHAIN: w_s / w_p already sit in registers
@@ -538,12 +571,12 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                         outs = us;
                     }
 
-                    store_state<UNIT>(a.v, os, vs[q]);
-                    store_state<UNIT>(a.w, wos, outs);
+                    store_state<UNIT>(a.v, os, vs[q], keep);
+                    store_state<UNIT>(a.w, wos, outs, keep);
                     if constexpr (PAIRED) {
-                        store_state<UNIT>(a.v, op, vp[q]);
+                        store_state<UNIT>(a.v, op, vp[q], keep);
                         if constexpr (!ONE_STORE)       // pair members keep separate copies
-                            store_state<UNIT>(a.w, wop, MODE == kPair ? outs : outp);
+                            store_state<UNIT>(a.w, wop, MODE == kPair ? outs : outp, keep);
                     }
 
                     if constexpr (DIAG) {
@@ -557,9 +590,9 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
                     }
                 }
                 if constexpr (EMIT) {     // outside `live`: the lanes of a warp shuffle together
-                    store_bf16<UNIT>(a.wb, wos, outs, live[q]);
+                    store_bf16<UNIT>(a.wb, wos, outs, live[q], keep);
                     if constexpr (PAIRED && !ONE_STORE)
-                        store_bf16<UNIT>(a.wb, wop, MODE == kPair ? outs : outp, live[q]);
+                        store_bf16<UNIT>(a.wb, wop, MODE == kPair ? outs : outp, live[q], keep);
                 }
             }
         }
@@ -627,8 +660,9 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
         const unsigned nb = gridDim.x;
         const int lane = tid & 31, warp = tid >> 5;
         for (int j = static_cast<int>(nb - 1u - blockIdx.x); j < a.n_work; j += static_cast<int>(nb)) {
-            const unsigned long long first = CHAIN ? 0ull : TILE_MAJOR ? static_cast<unsigned long long>(j)
-                                                   : static_cast<unsigned long long>(j) * static_cast<unsigned long long>(n_tiles);
+            const int jw = a.reverse ? a.n_work - 1 - j : j;   // position of item j in the walk
+            const unsigned long long first = CHAIN ? 0ull : TILE_MAJOR ? static_cast<unsigned long long>(jw)
+                                                   : static_cast<unsigned long long>(jw) * static_cast<unsigned long long>(n_tiles);
             const unsigned long long step1 = TILE_MAJOR ? static_cast<unsigned long long>(a.n_work) : 1ull;
             for (int k = warp; k < NQ; k += WARPS) {
                 const int row = j * NQ + k;

@@ -624,7 +624,7 @@ def test_max_S_unmixed_diagnostics_span_several_launches(H, oracle_mod):
 def test_diagnostics_stress_large_grids(H, oracle_mod):
     """Many work items (S = 32: 16 pairs, so several warps write block partials), the largest
     persistent grid (16 blocks/SM), many steps: diagnostics must equal the oracle's every step and be
-    bitwise identical between two runs (the ticketed last-block reduction has a fixed order)."""
+    bitwise identical between two runs (the collectors add the tagged block partials in a fixed order)."""
     from fixtures import problem
     S, G, P, seed, steps = 32, 2, 40_003, 181, 12
     runs = []
@@ -644,6 +644,61 @@ def test_diagnostics_stress_large_grids(H, oracle_mod):
         runs.append(np.stack(rec))
         h.close()
     assert np.array_equal(runs[0], runs[1])
+
+
+def test_diagnostics_under_graph_replay_with_fresh_gradients(H, oracle_mod, torch_cuda):
+    """A replayed graph re-launches the step with the SAME tag on its block partials.  The gradients
+    are refilled between replays, so a collector that picked up a partial of an earlier replay (a slot
+    it failed to zero) would report that replay's sums: every replay's diagnostics must equal the
+    oracle's for that step.  Several blocks per item and several items per collector-less block."""
+    torch = torch_cuda
+    from fixtures import problem
+    S, G, P, seed = 8, 2, 300_011, 77
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        h = H.Hadpsgd(S, G, [P], H.F32, H.DETERMINISTIC, stream=side)
+        problem.fill_weights(h, seed)
+        problem.fill_grads(h, seed, 0)
+    side.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        h.hadpsgd_step(LR, MU, 0)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    for rep in range(6):
+        with torch.cuda.stream(side):
+            problem.fill_grads(h, seed, rep)
+            graph.replay()
+            gd = h.hadpsgd_diagnostics()
+        od = oracle_mod.step(problem.host_grads(seed, rep, S, G, 0, P), ow, ov, LR, MU, 0, diag=True)
+        assert_diag(gd, od, rep)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    assert_parity(gw, gv, ow, ov, True)
+    h.close()
+
+
+def test_diagnostics_with_the_launch_shape_changing_every_step(H, oracle_mod):
+    """One handle, the grid and the number of work items changing from step to step (blocks per SM 1,
+    16, 3, default; matchings with 3, 1, 0 and 2 pairs): the block partials of one launch must never
+    be taken for those of another (different rows per block, different contributors per item)."""
+    from fixtures import problem
+    S, G, P, seed = 7, 3, 150_001, 191
+    seqs = [[1, 0, 3, 2, 5, 4, 6], [0, 1, 6, 3, 4, 5, 2], list(range(7)), [4, 1, 5, 3, 0, 2, 6]]
+    bps = [1, 16, 3, 0]
+    h = H.Hadpsgd(S, G, [P], H.F32, 0)
+    problem.fill_weights(h, seed)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    for k in range(12):
+        m = np.asarray(seqs[k % 4], np.int32)
+        h.hadpsgd_set_launch(bps[(k // 4 + k) % 4])
+        problem.fill_grads(h, seed, k)
+        h.hadpsgd_step_matching(LR, MU, k, m)
+        od = oracle_mod.step(problem.host_grads(seed, k, S, G, 0, P), ow, ov, LR, MU, k, diag=True, partner=m)
+        assert_diag(h.hadpsgd_diagnostics(), od, k)
+    gw = np.stack([h.hadpsgd_weights(s)[:P].cpu().numpy() for s in range(S)])
+    gv = np.stack([h.hadpsgd_momentum(s)[:P].cpu().numpy() for s in range(S)])
+    assert_parity(gw, gv, ow, ov, False)
+    h.close()
 
 
 @pytest.mark.parametrize("share", [False, True])
