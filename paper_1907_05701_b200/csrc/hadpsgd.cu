@@ -35,6 +35,7 @@ struct hadpsgd_ctx {
     bool walk_reverse = false;             // direction of the kernel's walk; flips with every step (L2 reuse)
     bool serpentine = true;
     size_t keep_bytes = size_t(64) << 20;  // bytes stored at the end of a step's walk that stay in L2
+    bool in_host_step = false;             // hadpsgd_step_host is enqueuing (its launches follow event waits)
     bool use_pdl = true;                   // launch steps with programmatic stream serialization
     uint32_t diag_tag = 0;                 // tag of the block partials of the most recent launch (never 0)
     uint64_t last_step_k = 0;
@@ -194,7 +195,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = h->use_pdl ? 1 : 0;
+    cfg.numAttrs = (h->use_pdl && !h->in_host_step) ? 1 : 0;   // chunk launches wait on copy events: plain launches
     CUDA_TRY(h, cudaLaunchKernelExC(&cfg, plan.fn, params));
     h->launches++;
     return HADPSGD_OK;
@@ -485,6 +486,8 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
     CUDA_TRY_DRAIN(cudaEventRecord(h->chunk_events[n_chunks], h->stream));
     CUDA_TRY_DRAIN(cudaStreamWaitEvent(h->copy_stream, h->chunk_events[n_chunks], 0));
     char* gdev = h->arena + h->L.g_off;
+    struct HostStepScope { hadpsgd_ctx* h; ~HostStepScope() { h->in_host_step = false; } } scope{h};
+    h->in_host_step = true;
     for (int c = 0; c < n_chunks; ++c) {
         const int64_t e0 = c * chunk, e1 = (e0 + chunk < P) ? e0 + chunk : P;
         for (int b = 0; b < n_buf; ++b)
