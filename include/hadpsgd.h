@@ -162,7 +162,13 @@ int hadpsgd_destroy(hadpsgd_handle h);
  * S odd and > 1 admits no perfect ring matching (R8): INVALID_ARG unless the handle
  * was created with HADPSGD_NO_MIX -- use hadpsgd_step_matching with an unpaired member instead.
  * Gradient buffers are read-only to the step (not zeroed); w and v are updated in place.
- * step_k is used only for its parity (no hidden counter: a step can be replayed).           */
+ * step_k is used only for its parity (no hidden counter: a step can be replayed).
+ * Launch: the kernel is launched with programmatic stream serialization and waits on the device
+ * (griddepcontrol.wait) for the operation before it on the stream, so the usual stream order holds
+ * towards every other kernel, copy or event; only capturable into a CUDA graph with a driver that
+ * knows programmatic dependencies (CUDA >= 12.3).  The direction of the kernel's walk over the
+ * buffers alternates from step to step (L2 reuse): w and v do not depend on it,
+ * the diagnostics only in the order their double-precision partial sums are added.             */
 int hadpsgd_step(hadpsgd_handle h, float lr, float momentum, uint64_t step_k);
 
 /* Same step, but with a caller-supplied matching (row f1): partner[s] must satisfy

@@ -125,7 +125,9 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     a.accumulate_diag = accumulate ? 1 : 0;
     a.reverse = h->walk_reverse ? 1 : 0;
     a.S = h->L.S;
-    a.partials = h->d_partials; a.diag = h->d_diag; a.tag = ++h->diag_tag ? h->diag_tag : ++h->diag_tag;
+    a.partials = h->d_partials; a.diag = h->d_diag;
+    if (++h->diag_tag == 0) h->diag_tag = 1;   // a tag is never 0 (zero = empty slot)
+    a.tag = h->diag_tag;
     for (int j = 0; j < n_items; ++j) {
         const WorkItem& it = items[j];
         a.items[j] = {static_cast<unsigned short>(it.s), static_cast<unsigned short>(it.p),
