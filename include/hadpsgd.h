@@ -270,7 +270,8 @@ int hadpsgd_plan_peer(int world, int rank, const int32_t* rank_begin, const int3
                       int32_t* write_buf, int32_t* read_peer);
 
 /* Measurement knob: resident blocks per SM of the persistent grid (1..16, clamped to what fits);
- * 0 restores the default chosen per (G, dtype, mode).  Results do not depend on it.          */
+ * 0 restores the default chosen per (G, dtype, mode).  w and v do not depend on it; the diagnostics
+ * only in the order their partial sums are added (same shape, same bits).                     */
 int hadpsgd_set_launch(hadpsgd_handle h, int blocks_per_sm);
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int hadpsgd_launch_count(hadpsgd_handle h, uint64_t* out);
