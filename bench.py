@@ -416,8 +416,19 @@ def time_e2e_steps(torch, dist, h, cfg, steps, warmup=1):
         dist.barrier()
     dev = ev0.elapsed_time(ev1) / 1e3
     assert d["gsq"].shape[0] == S
+    # what the link itself delivers on this box: the same pinned buffers copied to the gradient region with
+    # nothing else running (outside the timed region; the gradients on the device are left as they were)
+    link = None
+    if world == 1:
+        pairs = [(h.hadpsgd_grads(b // G if n_host == S * G else 0, b % G).view(torch.uint8), host[b]) for b in range(min(n_host, 8))]
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for dst, src in pairs:
+            dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+        link = len(pairs) * nbytes / (time.perf_counter() - t0) / 1e9
     note = f"{n_host} distinct pinned host buffers of {nbytes} B"
-    return max(dev, wall), S * G * nbytes, 3 * S * 8, note
+    return max(dev, wall), S * G * nbytes, 3 * S * 8, note, link
 
 
 def make_problem(H, torch, dist, args, cfg, flags, local, rank, world):
@@ -591,8 +602,7 @@ def run_ours(args):
 
     e2e = None
     if not args.no_e2e and not info.get("barrier"):
-        e_secs, h2d, d2h, note = time_e2e_steps(torch, dist, h, cfg, args.e2e_steps)
-        e2e = (e_secs, h2d, d2h, note)
+        e2e = time_e2e_steps(torch, dist, h, cfg, args.e2e_steps)   # (seconds, h2d bytes, d2h bytes, note, plain link GB/s)
 
     # max over ranks (device time), units and diagnostics summed over the ranks
     units = info["units"]
@@ -699,6 +709,7 @@ def run_ours(args):
             line["e2e"] = {"value": units / e_step, "unit": UNIT, "h2d_bytes_per_step": e2e[1],
                            "d2h_bytes_per_step": e2e[2], "ms_per_step": e_step * 1e3, "steps": args.e2e_steps,
                            "h2d_gbs": h2d_gbs, "frac_of_pcie_gen5_x16": h2d_gbs / PCIE_GEN5_X16_GBS,
+                           "link_gbs_plain_copy": e2e[4], "frac_of_plain_copy": (h2d_gbs / e2e[4]) if e2e[4] else None,
                            "note": "hadpsgd_step_host: " + e2e[3] + "; bound by the host-to-device copy of the S*G gradient "
                                    f"buffers (PCIe Gen5 x16, {PCIE_GEN5_X16_GBS:.0f} GB/s nominal per direction), which the "
                                    "fused kernel overlaps chunk by chunk; the new weights and momenta stay resident in HBM "
