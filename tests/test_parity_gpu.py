@@ -701,6 +701,58 @@ def test_diagnostics_with_the_launch_shape_changing_every_step(H, oracle_mod):
     h.close()
 
 
+def test_handles_stepping_concurrently_on_their_own_streams(H, torch_cuda):
+    """Four handles of different shapes (one with the largest grid, 16 blocks/SM) enqueue 60 steps each
+    on four streams at once, so their grids share the SMs and no grid is resident as a whole all the time:
+    the collectors of the diagnostics still get every block partial (they wait for blocks that are
+    running or queued, never for one that cannot run), and weights and diagnostics equal, bit for bit,
+    those of the same handles stepped one after the other."""
+    torch = torch_cuda
+    from fixtures import problem
+    shapes = [(16, 4, 300_011), (8, 8, 200_003), (4, 2, 1_000_003), (32, 2, 40_003)]
+
+    def run(concurrent, steps=60):
+        streams = [torch.cuda.Stream() for _ in shapes]
+        hs = []
+        for i, (S, G, P) in enumerate(shapes):
+            with torch.cuda.stream(streams[i]):
+                h = H.Hadpsgd(S, G, [P], H.F32, 0, stream=streams[i])
+                if i == 3:
+                    h.hadpsgd_set_launch(16)
+                problem.fill_weights(h, 50 + i)
+                problem.fill_grads(h, 50 + i, 0)
+            hs.append(h)
+        torch.cuda.synchronize()
+        recs = [[] for _ in hs]
+
+        def look(i):
+            d = hs[i].hadpsgd_diagnostics()
+            recs[i].append(np.concatenate([d["gsq"], d["wsq"], d["gap"]]))
+        if concurrent:
+            for k in range(steps):
+                for h in hs:
+                    h.hadpsgd_step(LR, MU, k)
+                if k % 20 == 19:
+                    for i in range(len(hs)):
+                        look(i)
+        else:
+            for i, h in enumerate(hs):
+                for k in range(steps):
+                    h.hadpsgd_step(LR, MU, k)
+                    if k % 20 == 19:
+                        look(i)
+        torch.cuda.synchronize()
+        out = [(np.stack(r), torch.stack([h.hadpsgd_weights(s) for s in range(h.S)]).cpu().numpy()) for r, h in zip(recs, hs)]
+        for h in hs:
+            h.close()
+        return out
+
+    serial, together = run(False), run(True)
+    for (d0, w0), (d1, w1) in zip(serial, together):
+        assert not np.isnan(d0).any() and np.array_equal(d0, d1)
+        assert np.array_equal(bits(w0), bits(w1))
+
+
 @pytest.mark.parametrize("share", [False, True])
 def test_host_gradient_path_equals_resident_path(H, oracle_mod, share):
     """hadpsgd_step_host (the e2e entry): chunked H2D + kernel on element sub-ranges must give
