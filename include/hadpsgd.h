@@ -223,6 +223,42 @@ int hadpsgd_set_diagnostics(hadpsgd_handle h, int enable);
  * synchronises the stream.  D_out: host.  Identity: D(u) - D(w') = 1/2 sum_pairs gap.         */
 int hadpsgd_consensus(hadpsgd_handle h, double* D_out);
 
+/* Consensus distance WITHOUT any allocation -- for callers that cannot give this library device memory.
+ * hadpsgd_consensus() above needs a handle, and a handle needs an arena (library-cudaMalloc'ed or carved
+ * out by the caller).  That is not always possible where D is wanted: the process's framework allocator
+ * may already hold nearly all of the GPU (a raw cudaMalloc then fails although the framework has room);
+ * a monitor between two steps of a latency-bound loop must not call cudaMalloc / cudaFree, which stall
+ * every stream of the device; a hook may only borrow S weight tensors and own no arena at all.  This
+ * entry point serves them: it takes the S weight buffers as plain device pointers and writes D to a
+ * device double, and its only scratch (one partial sum per thread block + a counter) is a fixed array
+ * inside the library image -- HADPSGD_NOALLOC_SCRATCH_BYTES on every GPU that loads the library, held
+ * until the process exits.  It calls no cudaMalloc, cudaFree or other allocating routine, on the device
+ * or on the host.
+ *   w       host array [S] of DEVICE pointers, each to n floats, 16-byte aligned, readable from the
+ *           CURRENT device (the call runs on the current device; it does not switch devices)
+ *   n       elements per buffer, 0 <= n <= HADPSGD_NOALLOC_MAX_ELEMS; need not be a multiple of 4
+ *   D_out   DEVICE pointer to one double (8-byte aligned); written by the kernel, in stream order
+ *   stream  cudaStream_t (NULL = legacy default stream); the call only enqueues and returns
+ * Same arithmetic as hadpsgd_consensus (mean and deviations in double, fixed summation order): for the
+ * same buffers the two agree to the last bit whenever the grids agree (#SMs x 8 <= MAX_BLOCKS blocks).
+ * Limits: S > HADPSGD_NOALLOC_MAX_S or n > HADPSGD_NOALLOC_MAX_ELEMS is INVALID_ARG, as are NULL,
+ * misaligned or plain-host pointers; the scratch bounds the GRID (HADPSGD_NOALLOC_MAX_BLOCKS), so no n
+ * within the limit is refused for lack of scratch.  Text of the last failure on the calling thread:
+ * hadpsgd_consensus_noalloc_error().
+ *   First call on a device: looks up the device address of the scratch array (cudaGetSymbolAddress) and
+ * clears its counter on `stream`; make that call outside any stream capture.  Later calls do neither.
+ *   Sharing: every call on a device uses the SAME scratch.  Calls are safe back to back on one stream
+ * (or otherwise ordered); two calls whose kernels may overlap on the GPU (different streams, threads or
+ * graphs without a dependency) race on it and give garbage -- serialise them.  Each call leaves the
+ * counter at zero and overwrites the partials it reads, so nothing has to be cleared in between.      */
+#define HADPSGD_NOALLOC_MAX_S 64
+#define HADPSGD_NOALLOC_MAX_BLOCKS 2048
+#define HADPSGD_NOALLOC_SCRATCH_BYTES ((HADPSGD_NOALLOC_MAX_BLOCKS + 32) * 8) /* 16,640 B per GPU */
+#define HADPSGD_NOALLOC_MAX_ELEMS ((int64_t)1 << 36)
+int hadpsgd_consensus_noalloc(const float* const* w /*host [S] of dev*/, int S, int64_t n,
+                              double* D_out /*dev*/, void* stream);
+const char* hadpsgd_consensus_noalloc_error(void);
+
 /* super-learner partition (row f4; Fig. 3) -------------------------------------
  * The paper's topology: every node holds ONE super-learner group and exchanges weights with its ring
  * neighbours.  Here `world` handles ("ranks": one per GPU and process, or several on one device),

@@ -77,6 +77,9 @@ def lib():
         L.hadpsgd_unshare.argtypes = [vp]
         L.hadpsgd_plan_slots.argtypes = [i32, i32p, i32, i32p, i32p, i32p, i32p, i32p, i32p]
         L.hadpsgd_consensus.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        L.hadpsgd_consensus_noalloc.argtypes = [ctypes.POINTER(vp), i32, ctypes.c_int64, vp, vp]
+        L.hadpsgd_consensus_noalloc_error.argtypes = []
+        L.hadpsgd_consensus_noalloc_error.restype = ctypes.c_char_p
         L.hadpsgd_peer_init.argtypes = [vp, i32, i32, i32p]
         L.hadpsgd_peer_stage.argtypes = [vp, ctypes.POINTER(vp)]
         L.hadpsgd_peer_attach.argtypes = [vp, i32, vp]
@@ -170,6 +173,21 @@ def hadpsgd_plan_peer(world, rank, rank_begin, partner, epoch, pending):
     d = {n: list(o) for n, o in zip(names, outs)}
     d["pending"] = list(pend)
     return d
+
+
+def hadpsgd_consensus_noalloc(weight_ptrs, n, out_ptr, stream_ptr=0):
+    """Consensus distance of S borrowed weight buffers, for callers that cannot let the library allocate
+    (a framework allocator that already holds the GPU, a monitor that must not stall the device with
+    cudaMalloc, a hook without an arena): see include/hadpsgd.h.  weight_ptrs: S device addresses of n
+    floats each; out_ptr: device address of one double, written in stream order; stream_ptr: a
+    cudaStream_t as int.  Marshalling only -- nothing is allocated here either.  Calls that may overlap
+    on the GPU share one scratch array and race; the first call on a device must be outside capture."""
+    S = len(weight_ptrs)
+    arr = (ctypes.c_void_p * max(S, 1))(*[int(p) for p in weight_ptrs])
+    L = lib()
+    rc = L.hadpsgd_consensus_noalloc(arr, S, int(n), ctypes.c_void_p(int(out_ptr)), ctypes.c_void_p(int(stream_ptr)))
+    if rc != OK:
+        raise HadpsgdError(rc, f"{L.hadpsgd_error_string(rc).decode()}: {L.hadpsgd_consensus_noalloc_error().decode()}")
 
 
 class Hadpsgd:

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhadpsgd.so")
-SOURCES = ["hadpsgd.cu", "step_f32.cu", "step_bf16.cu", "step_f32_emit.cu", "step_bf16_emit.cu", "consensus.cu", "peer_flush.cu",
+SOURCES = ["hadpsgd.cu", "step_f32.cu", "step_bf16.cu", "step_f32_emit.cu", "step_bf16_emit.cu", "consensus.cu", "consensus_noalloc.cu", "peer_flush.cu",
            "allocator.cpp", "scheduler.cpp", "schedule.cpp"]
 DEPS = SOURCES + ["internal.h", "step_kernel.cuh", "step_dispatch.cuh", os.path.join("..", "..", "include", "hadpsgd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
