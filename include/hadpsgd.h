@@ -288,10 +288,17 @@ int hadpsgd_peer_stage(hadpsgd_handle h, float** dev_ptr);
  * rank other than the handle's own must be attached before the first step.                       */
 int hadpsgd_peer_attach(hadpsgd_handle h, int r, const float* stage_region_of_rank_r);
 /* Across processes: export this handle's arena as a CUDA IPC handle (ipc_handle_out: host, 64 bytes)
- * plus the byte offset of the stage region from the exported allocation's base ...                 */
+ * plus the byte offset of the stage region from the exported allocation's base ...
+ * A CUDA IPC handle names a whole ALLOCATION, so the importing process can read everything that
+ * shares the arena's cudaMalloc block.  Create handles that will be exported with opts->arena = NULL
+ * (library-owned: the allocation is exactly the arena) or over a dedicated cudaMalloc of your own.  A
+ * slice of a framework's caching allocator exposes that allocator's whole segment to the peer -- unrelated
+ * tensors included -- and memory from cudaMallocAsync pools or virtual-memory ("expandable") segments
+ * cannot be exported this way at all (cudaIpcGetMemHandle fails: HADPSGD_CUDA).                      */
 int hadpsgd_peer_ipc_export(hadpsgd_handle h, void* ipc_handle_out, uint64_t* stage_offset_out);
 /* ... and open rank r's export in this process (cudaIpcOpenMemHandle with lazy peer access), then
- * attach it.  The mapping is closed by hadpsgd_destroy().                                           */
+ * attach it.  One mapping per rank: attaching rank r again synchronises the stream, closes r's
+ * previous mapping and opens the new one; hadpsgd_destroy() closes what is left.                    */
 int hadpsgd_peer_ipc_attach(hadpsgd_handle h, int r, const void* ipc_handle, uint64_t stage_offset);
 /* Materialise every pending mix: w_s = 1/2 (u_own + u_partner) into the main weight buffer (one small
  * kernel on the stream; asynchronous), delivering pend_wsq / pend_gap.  Call after the epoch barrier.

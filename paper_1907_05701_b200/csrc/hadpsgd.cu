@@ -33,10 +33,10 @@ struct hadpsgd_ctx {
     double* d_scratch = nullptr;           // consensus / flush kernels: block partials, plain doubles
     double* d_diag = nullptr;
     bool walk_reverse = false;             // direction of the kernel's walk; flips with every step (L2 reuse)
-    bool serpentine = true;
-    size_t keep_bytes = size_t(64) << 20;  // bytes stored at the end of a step's walk that stay in L2
+    const bool serpentine = true;          // fixed choices of the build: nothing is read from the environment
+    const size_t keep_bytes = size_t(64) << 20;  // bytes stored at the end of a step's walk that stay in L2
     bool in_host_step = false;             // hadpsgd_step_host is enqueuing (its launches follow event waits)
-    bool use_pdl = true;                   // launch steps with programmatic stream serialization
+    const bool use_pdl = true;             // launch steps with programmatic stream serialization
     uint32_t diag_tag = 0;                 // tag of the block partials of the most recent launch (never 0)
     uint64_t last_step_k = 0;
     int last_n_pairs = 0;
@@ -44,7 +44,10 @@ struct hadpsgd_ctx {
     int blocks_per_sm = 0;   // tuning override of the persistent grid (0 = the plan's default)
     bool diag_on = true;     // hadpsgd_set_diagnostics: a5 computed by the steps that follow (never with NO_DIAG)
     uint64_t diag_step_k = 0;   // step_k of the most recent step that computed diagnostics
-    std::vector<int32_t> partner;   // scratch of the step calls (no allocation per step)
+    // scratch of the step calls: sized by the first step, reused afterwards (no host allocation per step)
+    std::vector<int32_t> partner, new_slot, new_pending;
+    std::vector<SlotCopy> copies;
+    std::vector<WorkItem> part[2][2];   // peer mode: [pairs | singles][plain | pending]
     StepPlan plan;
     // super-learner partition (HADPSGD_PEER)
     bool peer_init = false, peer_table_dirty = true;
@@ -54,7 +57,7 @@ struct hadpsgd_ctx {
     std::vector<int32_t> pending;              // [S] global partner whose stage completes w_s, or -1
     uint64_t epoch = 0;
     const float** d_peer = nullptr;            // device table [2][S_global]
-    std::vector<void*> ipc_mapped;             // cudaIpcOpenMemHandle results, closed at destroy
+    std::vector<void*> ipc_mapped;             // [world] the cudaIpcOpenMemHandle mapping of rank r (nullptr: none); closed on re-attach and at destroy
     std::string err;
 };
 
@@ -74,7 +77,7 @@ int launch_consensus(const float* w, long long P_padded, int S, const int32_t* w
                      double* block_out, cudaStream_t stream, cudaError_t* err);   // consensus.cu
 int launch_peer_flush(float* w_main, const float* a_stage, const float* const* peer, const int32_t* members,
                       int n_members, long long P_padded, int S, int num_sms, double* partials, double* diag,
-                      bool exact, cudaStream_t stream, cudaError_t* err);         // peer_flush.cu
+                      cudaStream_t stream, cudaError_t* err);                     // peer_flush.cu
 }
 
 // ---- kernel dispatch -------------------------------------------------------------------
@@ -233,12 +236,12 @@ int step_range(hadpsgd_ctx* h, const StepPlan& sp, float lr, float mu, int64_t e
     // item's buffer indices anyway.  The plain kernels do not know pend_wsq / pend_gap: clear them.
     if (!(h->flags & HADPSGD_NO_DIAG) && h->diag_on && !accumulate)
         CUDA_TRY(h, cudaMemsetAsync(h->d_diag + 3 * h->L.S, 0, sizeof(double) * 2 * h->L.S, h->stream));
-    std::vector<WorkItem> part[2][2];   // [pairs | singles][plain | pending]
-    for (const WorkItem& it : sp.pairs) part[0][(it.b_s || it.b_p) ? 1 : 0].push_back(it);
-    for (const WorkItem& it : sp.singles) part[1][it.b_s ? 1 : 0].push_back(it);
+    for (auto& row : h->part) for (auto& v : row) v.clear();   // [pairs | singles][plain | pending]
+    for (const WorkItem& it : sp.pairs) h->part[0][(it.b_s || it.b_p) ? 1 : 0].push_back(it);
+    for (const WorkItem& it : sp.singles) h->part[1][it.b_s ? 1 : 0].push_back(it);
     for (int kind = 0; kind < 2; ++kind)
         for (int pend = 0; pend < 2; ++pend) {
-            int rc = launch_items(h, part[kind][pend], kind == 0 ? kPair : kSingle, pend ? kPeer : kOwn, lr, mu,
+            int rc = launch_items(h, h->part[kind][pend], kind == 0 ? kPair : kSingle, pend ? kPeer : kOwn, lr, mu,
                                   elem_begin, elem_end, accumulate);
             if (rc != HADPSGD_OK) return rc;
         }
@@ -295,11 +298,11 @@ int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp, std::
         return HADPSGD_OK;
     }
     const bool share = h->flags & HADPSGD_SHARE_PAIR_WEIGHTS;
-    std::vector<SlotCopy> copies;
+    h->copies.clear();
     *new_slot = h->w_slot;
-    plan_step(h->L.S, partner, share, new_slot, &sp->pairs, &sp->singles, &copies);
+    plan_step(h->L.S, partner, share, new_slot, &sp->pairs, &sp->singles, &h->copies);
     sp->shared = share;
-    return copy_slots(h, copies);
+    return copy_slots(h, h->copies);
 }
 
 void commit_plan(hadpsgd_ctx* h, const StepPlan& sp, const std::vector<int32_t>& new_slot,
@@ -377,9 +380,6 @@ extern "C" int hadpsgd_create(int S, int G, const int64_t* seg_len, int n_seg, h
         if (!dt.peer_stage) { g_create_error = "HADPSGD_PEER needs dtypes.peer_stage = 1 (the stage buffers)"; return HADPSGD_INVALID_ARG; }
     }
     hadpsgd_ctx* h = new hadpsgd_ctx();
-    if (const char* e_pdl = std::getenv("HADPSGD_PDL")) h->use_pdl = e_pdl[0] != '0';   // development switch
-    if (const char* e_sp = std::getenv("HADPSGD_SERPENTINE")) h->serpentine = e_sp[0] != '0';   // development switch
-    if (const char* e_kb = std::getenv("HADPSGD_KEEP_MB")) h->keep_bytes = static_cast<size_t>(std::atoll(e_kb)) << 20;   // development switch
     h->w_slot.resize(S);
     for (int s = 0; s < S; ++s) h->w_slot[s] = s;
     h->pending.assign(S, -1);
@@ -418,7 +418,7 @@ extern "C" int hadpsgd_destroy(hadpsgd_handle h) {
     for (cudaEvent_t ev : h->chunk_events) cudaEventDestroy(ev);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     if (h->d_peer) cudaFree(h->d_peer);
-    for (void* p : h->ipc_mapped) cudaIpcCloseMemHandle(p);
+    for (void* p : h->ipc_mapped) if (p) cudaIpcCloseMemHandle(p);
     if (h->owns_arena) cudaFree(h->arena);
     delete h;
     return HADPSGD_OK;
@@ -434,12 +434,11 @@ extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum,
     DeviceGuard guard(h->device);
     int rc = build_partner(h, step_k, partner, &h->partner);
     if (rc != HADPSGD_OK) return rc;
-    std::vector<int32_t> new_slot, new_pending;
-    rc = plan_and_prepare(h, h->partner.data(), &h->plan, &new_slot, &new_pending);
+    rc = plan_and_prepare(h, h->partner.data(), &h->plan, &h->new_slot, &h->new_pending);
     if (rc != HADPSGD_OK) return rc;
     rc = step_range(h, h->plan, lr, momentum, 0, h->L.P_padded, false);
     if (rc != HADPSGD_OK) return rc;
-    commit_plan(h, h->plan, new_slot, new_pending, step_k);   // only now: every launch is enqueued
+    commit_plan(h, h->plan, h->new_slot, h->new_pending, step_k);   // only now: every launch is enqueued
     return HADPSGD_OK;
 }
 
@@ -465,7 +464,8 @@ extern "C" int hadpsgd_step_host(hadpsgd_handle h, const void* const* host_grads
         h->chunk_events.push_back(ev);
     }
 
-    std::vector<int32_t> new_slot, new_pending;    // one slot plan for the whole step, shared by all chunks
+    std::vector<int32_t>& new_slot = h->new_slot;  // one slot plan for the whole step, shared by all chunks
+    std::vector<int32_t>& new_pending = h->new_pending;
     rc = plan_and_prepare(h, h->partner.data(), &h->plan, &new_slot, &new_pending);
     if (rc != HADPSGD_OK) return rc;
 
@@ -608,6 +608,8 @@ extern "C" int hadpsgd_peer_init(hadpsgd_handle h, int rank, int world, const in
                  std::to_string(rank_begin[rank + 1] - rank_begin[rank]);
         return HADPSGD_INVALID_ARG;
     }
+    for (void* p : h->ipc_mapped) if (p) cudaIpcCloseMemHandle(p);   // a repeated init (before the first step) starts over
+    h->ipc_mapped.assign(world, nullptr);
     h->rank = rank; h->world = world; h->S_global = rank_begin[world];
     h->rank_begin.assign(rank_begin, rank_begin + world + 1);
     h->stage_of_rank.assign(world, nullptr);
@@ -663,12 +665,22 @@ extern "C" int hadpsgd_peer_ipc_export(hadpsgd_handle h, void* ipc_handle_out, u
 extern "C" int hadpsgd_peer_ipc_attach(hadpsgd_handle h, int r, const void* ipc_handle, uint64_t stage_offset) {
     if (!h || !ipc_handle) return HADPSGD_INVALID_ARG;
     if (!is_peer(h) || !h->peer_init) { h->err = "call hadpsgd_peer_init first"; return HADPSGD_INVALID_ARG; }
+    if (r < 0 || r >= h->world || r == h->rank) { h->err = "rank out of range (or the handle's own rank)"; return HADPSGD_INVALID_ARG; }
     DeviceGuard guard(h->device);
+    if (h->ipc_mapped[r]) {
+        // re-attach: one mapping per rank.  No launch may still read through the old one.
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+        void* old_base = h->ipc_mapped[r];
+        h->ipc_mapped[r] = nullptr;
+        h->stage_of_rank[r] = nullptr;
+        h->peer_table_dirty = true;
+        CUDA_TRY(h, cudaIpcCloseMemHandle(old_base));
+    }
     cudaIpcMemHandle_t ipc;
     std::memcpy(&ipc, ipc_handle, sizeof ipc);
     void* base = nullptr;
     CUDA_TRY(h, cudaIpcOpenMemHandle(&base, ipc, cudaIpcMemLazyEnablePeerAccess));
-    h->ipc_mapped.push_back(base);
+    h->ipc_mapped[r] = base;
     return hadpsgd_peer_attach(h, r, reinterpret_cast<const float*>(static_cast<char*>(base) + stage_offset));
 }
 
@@ -687,8 +699,7 @@ extern "C" int hadpsgd_peer_flush(hadpsgd_handle h) {
     const float* a_stage = reinterpret_cast<const float*>(h->arena + h->L.stage_off) + static_cast<size_t>(rd) * h->L.S * h->L.P_padded;
     launch_peer_flush(reinterpret_cast<float*>(h->arena + h->L.w_off), a_stage, h->d_peer, members.data(),
                       static_cast<int>(members.size() / 2), h->L.P_padded, h->L.S, h->num_sms,
-                      ((h->flags & HADPSGD_NO_DIAG) || !h->diag_on) ? nullptr : h->d_scratch, h->d_diag,
-                      (h->flags & HADPSGD_DETERMINISTIC) != 0, h->stream, &e);
+                      ((h->flags & HADPSGD_NO_DIAG) || !h->diag_on) ? nullptr : h->d_scratch, h->d_diag, h->stream, &e);
     CUDA_TRY(h, e);
     h->launches++;
     h->pending.assign(h->L.S, -1);

@@ -83,7 +83,7 @@ __global__ void flush_reduce_kernel(const __grid_constant__ FlushArgs a, int gri
 // members: n pairs (local member, peer-table entry).  Enqueues on `stream`.
 int launch_peer_flush(float* w_main, const float* a_stage, const float* const* peer, const int32_t* members,
                       int n_members, long long P_padded, int S, int num_sms, double* partials, double* diag,
-                      bool /*exact*/, cudaStream_t stream, cudaError_t* err) {
+                      cudaStream_t stream, cudaError_t* err) {
     *err = cudaSuccess;
     for (int first = 0; first < n_members && *err == cudaSuccess; first += kMaxFlush) {
         FlushArgs a;

@@ -487,6 +487,7 @@ def _ipc_worker(rank, world, port, out_dir):
             if r != rank:
                 raw = bytes(got[r].tolist())
                 h.hadpsgd_peer_ipc_attach(r, raw[:64], int.from_bytes(raw[64:], "little"))
+                h.hadpsgd_peer_ipc_attach(r, raw[:64], int.from_bytes(raw[64:], "little"))   # re-attach: the old mapping is closed
         for s in range(4):
             device.fill(h.hadpsgd_weights(s)[:P], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, lo + s, 0), "normal", 0.05)
         for k in range(steps):
