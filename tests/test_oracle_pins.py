@@ -702,3 +702,70 @@ def test_round_bf16_matches_library_and_fixed_points(oracle_mod):
     assert [int(v) for v in oracle_mod.round_bf16(sp)] == [0x7F80, 0xFF80, 0x7F80, 0xFF80, 0x0000, 0x8000]
     nan = oracle_mod.round_bf16(np.array([np.nan], np.float32))[0]
     assert (nan & 0x7F80) == 0x7F80 and (nan & 0x007F) != 0
+
+
+# ------------------------------------------------------------------ bf16 edge values (R6, R17)
+
+BF16_EDGE = [0x0000, 0x8000,             # +0, -0
+             0x0001, 0x007F, 0x8001,     # subnormal bf16: smallest, largest, negative smallest
+             0x0080, 0x8080,             # smallest normals
+             0x3F80, 0xBF80,             # +-1
+             0x7F7F, 0xFF7F,             # largest finite
+             0x7F80, 0xFF80,             # +-Inf
+             0x7FC0, 0xFFC1, 0x7F81]     # NaNs: quiet, negative with payload, quiet bit clear
+
+
+def test_bf16_gradient_widening_is_exact_on_edge_values(oracle_mod):
+    """R6 ("bf16 -> fp32 widening is exact") with R17 (no flush-to-zero) on the values a
+    Gaussian draw never produces.  S = 1, G = 1, mu = 0, lr = 1, w = v = 0: the mean is the gradient
+    itself (eq. (6) with one learner), so v' = 0*0 + g must be the widened gradient
+    (h << 16 as an fp32 pattern, built here) bit for bit and w' = 0 - 1*v' its negation -- down to the
+    smallest subnormal.  -0 is the one value the arithmetic itself changes: (+0) + (-0) = +0."""
+    h = np.array(BF16_EDGE, dtype=np.uint16)
+    want = (h.astype(np.uint32) << np.uint32(16)).view(np.float32)        # the definition of bf16
+    P = len(h)
+    for G in (1, 2):                        # G = 2: (g + 0) * 0.5 halves exactly unless it underflows
+        g = np.zeros((1, G, P), np.uint16)
+        g[0, 0] = h
+        w, v = np.zeros((1, P), np.float32), np.zeros((1, P), np.float32)
+        oracle_mod.step(g, w, v, 1.0, 0.0, 0)
+        with np.errstate(invalid="ignore"):
+            exp_v = want if G == 1 else (want.astype(np.float64) * 0.5).astype(np.float32)   # exact or RNE once: the definition
+        nan = np.isnan(want)
+        assert np.array_equal(np.isnan(v[0]), nan) and np.array_equal(np.isnan(w[0]), nan)
+        ok = ~nan & (h != 0x8000)
+        assert np.array_equal(bits(v[0][ok]), bits(exp_v[ok])), [hex(int(x)) for x in bits(v[0])]
+        assert np.array_equal(bits(w[0][ok]), bits(np.float32(0) - exp_v[ok]))        # 0 - 1*v': exact; (+0) - (+0) = +0
+        assert bits(v[0][h == 0x8000])[0] == 0 and bits(w[0][h == 0x8000])[0] == 0        # -0 -> +0 + -0 = +0
+        if G == 1:                          # the subnormals in particular: not flushed
+            assert [int(x) for x in bits(v[0][2:5])] == [0x00010000, 0x007F0000, 0x80010000]
+            assert v[0][2] > 0 and v[0][4] < 0
+    # the double-precision shadow widens the same way
+    g = np.zeros((1, 1, P), np.uint16)
+    g[0, 0] = h
+    w64, v64 = np.zeros((1, P)), np.zeros((1, P))
+    oracle_mod.step_f64(g, w64, v64, 1.0, 0.0, 0)
+    fin = np.isfinite(want)
+    assert np.array_equal(v64[0][fin], want[fin].astype(np.float64))
+
+
+def test_round_bf16_of_a_nan_is_a_nan_never_inf(oracle_mod):
+    """R17 reading for the bf16 working copy (row f2): a NaN weight rounds to A NaN -- which one (sign,
+    payload) is not specified, because the CUDA path's cvt.rn.bf16x2.f32 returns the canonical 0x7FFF
+    while this oracle keeps sign and upper payload -- so the tests compare NaN-ness.  What IS fixed:
+    never +-Inf (a NaN whose upper seven mantissa bits are zero must not truncate to 0x7F80), and
+    +-Inf / finite values are never turned into NaN."""
+    nan_bits = np.array([0x7F800001, 0xFF800001, 0x7F80FFFF, 0x7FC00000, 0xFFC00000, 0x7F8ABCDE, 0xFFFFFFFF,
+                         0x7FBFFFFF, 0x7F810000], dtype=np.uint32)
+    got = oracle_mod.round_bf16(nan_bits.view(np.float32))
+    for b, r in zip(nan_bits, got):
+        assert (int(r) & 0x7F80) == 0x7F80 and (int(r) & 0x007F) != 0, (hex(int(b)), hex(int(r)))
+    widened = (got.astype(np.uint32) << np.uint32(16)).view(np.float32)
+    assert np.isnan(widened).all()
+    # and nothing that is not a NaN becomes one: Inf, the overflow to Inf, the largest values that stay finite
+    sp = np.array([0x7F800000, 0xFF800000, 0x7F7FFFFF, 0xFF7FFFFF, 0x7F7F8000, 0x7F7F7FFF, 0x7F7F0000], dtype=np.uint32)
+    assert [int(x) for x in oracle_mod.round_bf16(sp.view(np.float32))] == [0x7F80, 0xFF80, 0x7F80, 0xFF80, 0x7F80, 0x7F7F, 0x7F7F]
+    # subnormal fp32 weights round among subnormal bf16 values (no flush): 0x00008000 is a tie -> even (0),
+    # 0x00018000 a tie -> even (2), 0x00008001 just above the tie -> 1
+    sub = np.array([0x00008000, 0x00018000, 0x00008001, 0x80008001, 0x007FFFFF], dtype=np.uint32)
+    assert [int(x) for x in oracle_mod.round_bf16(sub.view(np.float32))] == [0x0000, 0x0002, 0x0001, 0x8001, 0x0080]
