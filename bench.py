@@ -42,7 +42,7 @@ UNIT = "learner-params/s"
 LR, MU = 0.1, 0.9
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 PCIE_GEN5_X16_GBS = 64.0        # nominal per direction; the e2e leg reports its fraction of this
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r03_traffic.csv")
 KERNEL_SOURCES = ["paper_1907_05701_b200/csrc/step_kernel.cuh", "paper_1907_05701_b200/csrc/step_dispatch.cuh"]
 
 
@@ -57,7 +57,7 @@ def kernel_source_sha():
 
 def ncu_traffic(workload, flags_text, emit):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed
-    `ncu --set full` captures (profiles/r02_traffic.csv; the .md beside it names the commands).  Only a
+    `ncu --set full` captures (profiles/r03_traffic.csv; the .md beside it names the commands).  Only a
     capture taken on THIS kernel source (sha of step_kernel.cuh + step_dispatch.cuh) for this workload
     and these flags counts; anything else is None."""
     import csv
@@ -67,9 +67,9 @@ def ncu_traffic(workload, flags_text, emit):
             for row in csv.DictReader(f):
                 if (row["workload"], row["flags"], row["emit_bf16"]) == want:
                     if row["kernel_source_sha16"] != kernel_source_sha():
-                        return None, f"profiles/r02_traffic.csv holds a capture of another kernel source ({row['kernel_source_sha16']})"
+                        return None, f"profiles/r03_traffic.csv holds a capture of another kernel source ({row['kernel_source_sha16']})"
                     return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), \
-                        f"profiles/r02_traffic.csv: {row['kernel']} at commit {row['commit']} (read {row['dram_bytes_read']} B + write {row['dram_bytes_write']} B)"
+                        f"profiles/r03_traffic.csv: {row['kernel']} at commit {row['commit']} (read {row['dram_bytes_read']} B + write {row['dram_bytes_write']} B)"
     except Exception as e:                      # no capture file: say so, never guess
         return None, f"no capture: {e}"
     return None, "no capture for this workload / flags"
@@ -97,7 +97,9 @@ def parse_args():
     ap.add_argument("--emulate-ranks", type=int, default=0,
                     help="N = 1 only: time the super-learner partition over R HADPSGD_PEER handles on ONE GPU (one stream; "
                          "peer reads are local HBM reads) -- kernel cost of the partition, not an NVLink measurement")
-    ap.add_argument("--no-ceiling", action="store_true", help="skip the pure-read / pure-write membench legs")
+    ap.add_argument("--no-ceiling", action="store_true", help="skip the pure-read / pure-write membench legs (roofline.reference_mix)")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the device-timed legs of the other kernel families (`secondary`) and the bf16 e2e leg")
     ap.add_argument("--cpu-repeats", type=int, default=3)
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[4]: bandwidth sweep over P, S, G (one JSON line per point)")
@@ -528,17 +530,67 @@ def time_device_steps_barrier(torch, dist, h, steps, warmup, k0=0, sampler=None)
     return ev0.elapsed_time(ev1) / 1e3, clocks
 
 
-def mix_ceiling(torch, read_bytes, write_bytes):
+def reference_mix_rate(torch, read_bytes, write_bytes):
     """This box's pure-read and pure-write streaming rates (fixtures/membench.cu, the step kernel's access
-    shape) and the ceiling they imply for this kernel's byte mix: reads and writes share one DRAM bus, so
-    t >= read_bytes / BW_read + write_bytes / BW_write."""
+    shape) and the rate they imply for this kernel's byte mix if reads and writes simply took turns on the
+    DRAM bus: t = read_bytes / BW_read + write_bytes / BW_write.  A REFERENCE rate, not an upper bound: the
+    membench legs are one plain kernel each (one block per SM) and the step kernel has measured up to 3 %
+    above the figure, so a fraction slightly over 1 is not an inconsistency."""
     from fixtures import device
     r = device.membench(8 << 30, 12, write=False, reps=3)
     w = device.membench(8 << 30, 4, write=True, reps=3)
     t = read_bytes / (r * 1e9) + write_bytes / (w * 1e9)
     return {"read_gbs": r, "write_gbs": w, "mix_gbs": (read_bytes + write_bytes) / t / 1e9,
             "how": "fixtures/membench.cu: 12 read streams / 4 write streams, 32 B accesses, 148 x 256 threads, best of 3; "
-                   "mix = bytes / (read_bytes / read_gbs + write_bytes / write_gbs)"}
+                   "mix = bytes / (read_bytes / read_gbs + write_bytes / write_gbs); a reference rate for this byte mix, "
+                   "not an upper bound (the legs are untuned single kernels)"}
+
+
+def secondary_leg(H, torch, args, name, emit):
+    """One more kernel family, device-timed like the headline: BASELINE.json configs[3] (ragged bf16, 8 x 8),
+    the headline shape with the bf16 working copy (row f2), the paper-literal model (8 x 8 fp32)."""
+    from fixtures import problem
+    cfg = workload(name)
+    cfg["emit"] = emit
+    h = H.Hadpsgd(cfg["S"], cfg["G"], cfg["seg_len"], H.BF16 if cfg["grad"] == "bf16" else H.F32, 0, device=0,
+                  working_dtype=H.BF16 if emit else H.F32)
+    problem.fill_weights(h, 2000)
+    problem.fill_grads(h, 2000, 0, cfg["dist"])
+    torch.cuda.synchronize()
+    n0 = h.hadpsgd_launch_count()
+    secs, clocks = time_device_steps(torch, None, h, args.steps, args.warmup, sampler=ClockSampler(0))
+    launches = h.hadpsgd_launch_count() - n0 - args.warmup
+    t = secs / args.steps
+    abytes = cfg["S"] * h.P_padded * (cfg["G"] * cfg["b_g"] + 16 + (2 if emit else 0))
+    traffic, src = ncu_traffic(name, "", emit)
+    h.close()
+    del h
+    torch.cuda.empty_cache()
+    return {"workload": name, "working_dtype": "bf16" if emit else "f32", "S": cfg["S"], "G": cfg["G"], "P": cfg["P"],
+            "grad_dtype": cfg["grad"], "ms_per_step": t * 1e3, "value": cfg["S"] * cfg["G"] * cfg["P"] / t, "unit": UNIT,
+            "algorithmic_bytes_per_launch": abytes, "achieved_gbs": abytes / t / 1e9,
+            "frac_of_8TBps_nominal": abytes / t / 1e9 / 8000.0, "frac_of_measured_copy_peak": abytes / t / 1e9 / measured_peak()[0],
+            "traffic": traffic, "traffic_source": src, "gpu_launches": launches, "steps": args.steps, "warmup": args.warmup,
+            "clocks": clocks}
+
+
+def e2e_leg_bf16(H, torch, args):
+    """The end-to-end call (hadpsgd_step_host, pinned host gradients, copies inside the timed region) on the
+    bf16-gradient handle of configs[3]: half the PCIe bytes per learner-parameter of the fp32 headline."""
+    from fixtures import problem
+    cfg = workload("swb2000_ragged_bf16")
+    h = H.Hadpsgd(cfg["S"], cfg["G"], cfg["seg_len"], H.BF16, 0, device=0)
+    problem.fill_weights(h, 2000)
+    problem.fill_grads(h, 2000, 0, cfg["dist"])
+    torch.cuda.synchronize()
+    secs, h2d, d2h, note, link = time_e2e_steps(torch, None, h, cfg, args.e2e_steps)
+    h.close()
+    del h
+    torch.cuda.empty_cache()
+    e_step = secs / args.e2e_steps
+    return {"workload": "swb2000_ragged_bf16", "value": cfg["S"] * cfg["G"] * cfg["P"] / e_step, "unit": UNIT,
+            "ms_per_step": e_step * 1e3, "steps": args.e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "h2d_gbs": h2d / e_step / 1e9, "link_gbs_plain_copy": link, "note": "hadpsgd_step_host on bf16 gradients: " + note}
 
 
 def run_ours(args):
@@ -646,6 +698,17 @@ def run_ours(args):
         del hs
         torch.cuda.empty_cache()
 
+    # Device-timed legs of the other kernel families, beside the headline (never instead of it): same
+    # steps / warm-up, each with its own clock record.  Only on the default single-GPU headline run.
+    secondary = None
+    e2e_bf16 = None
+    if (world == 1 and dist is None and not args.no_secondary and args.workload == "swb2000" and not args.flags
+            and not args.emit_bf16 and not args.blocks_per_sm):
+        secondary = [secondary_leg(H, torch, args, name, emit) for name, emit in
+                     (("swb2000_ragged_bf16", False), ("swb2000", True), ("paper_literal", False))]
+        if not args.no_e2e:
+            e2e_bf16 = e2e_leg_bf16(H, torch, args)
+
     if rank == 0:
         t_step = secs / args.steps
         peak, peak_src = measured_peak()
@@ -659,7 +722,7 @@ def run_ours(args):
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes_rank,
                 "kernel": "hadpsgd::step_kernel (one launch = one step)", "frac_of_8TBps_nominal": achieved / 8000.0,
                 "note": "peak is a 1:1 copy; this kernel reads more than it writes, and reads are the faster direction, "
-                        "so frac may exceed 1 (see ceiling)"}
+                        "so frac may exceed 1 (see reference_mix)"}
         if "nvlink_read_bytes_per_rank_per_step" in info:
             # fused compute + peer-read kernel: the floor of a step is the slower of its local HBM bytes at the
             # measured HBM peak and its NVLink bytes at the measured peer-copy rate (B200_PROFILING.md: 770 GB/s)
@@ -671,9 +734,9 @@ def run_ours(args):
                               "note": "floor = max(local bytes / measured HBM peak, peer bytes / 770 GB/s) per step parity"}
         if not args.no_ceiling and world == 1:
             rd = S_rank * P_rank * (cfg["G"] * cfg["b_g"] + 8)
-            ceil = mix_ceiling(torch, rd, abytes_rank - rd)
-            ceil["frac_of_mix_ceiling"] = achieved / ceil["mix_gbs"]
-            roof["ceiling"] = ceil
+            ref = reference_mix_rate(torch, rd, abytes_rank - rd)
+            ref["frac_of_reference_mix_rate"] = achieved / ref["mix_gbs"]
+            roof["reference_mix"] = ref
         line = {
             "metric": METRIC, "value": units / t_step, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
@@ -714,6 +777,10 @@ def run_ours(args):
                                    f"buffers (PCIe Gen5 x16, {PCIE_GEN5_X16_GBS:.0f} GB/s nominal per direction), which the "
                                    "fused kernel overlaps chunk by chunk; the new weights and momenta stay resident in HBM "
                                    "(the learners live on the GPU), so the device-to-host traffic is the diagnostics only"}
+        if secondary is not None:
+            line["secondary"] = secondary
+        if e2e_bf16 is not None:
+            line["e2e_bf16"] = e2e_bf16
         if cpu_line is not None:
             line["cpu_baseline"] = cpu_line
         print(json.dumps(line), file=_REAL_STDOUT or sys.stdout, flush=True)

@@ -49,7 +49,8 @@ enum { /* status codes */
                                         hadpsgd_step with S odd and >1 (no perfect ring matching)      */
     HADPSGD_OUT_OF_MEMORY = -2,      /* arena too small / cudaMalloc failed                                */
     HADPSGD_CUDA = -3,               /* CUDA runtime or launch error; text via hadpsgd_last_error()        */
-    HADPSGD_UNSUPPORTED_DEVICE = -4  /* compute capability != 10.x: no multi-backend dispatch, no fallback */
+    HADPSGD_UNSUPPORTED_DEVICE = -4, /* compute capability != 10.x: no multi-backend dispatch, no fallback */
+    HADPSGD_DIAG_TIMEOUT = -5        /* hadpsgd_diagnostics only: see "Sharing the device" there          */
 };
 
 enum { /* hadpsgd_opts.flags */
@@ -158,7 +159,11 @@ int hadpsgd_destroy(hadpsgd_handle h);
 
 /* a2-a6 the step ----------------------------------------------------------------------------- */
 
-/* Enqueue one fused step (one kernel launch) on the handle's stream; asynchronous.
+/* Enqueue one fused step on the handle's stream; asynchronous.  Launches per step: ONE for the ring
+ * matching or any matching whose members are all paired or all unmixed (up to 32 pairs -- S <= 64 -- per
+ * launch); two for a matching that has both (pairs, then singles); on a HADPSGD_PEER handle up to four
+ * (pairs / singles, each split into members that first resolve a pending mix and members that do not),
+ * back to back with nothing in between.  hadpsgd_launch_count() counts them.
  * S odd and > 1 admits no perfect ring matching (R8): INVALID_ARG unless the handle
  * was created with HADPSGD_NO_MIX -- use hadpsgd_step_matching with an unpaired member instead.
  * Gradient buffers are read-only to the step (not zeroed); w and v are updated in place.
@@ -209,12 +214,23 @@ int hadpsgd_segment(hadpsgd_handle h, int seg, int64_t* elem_offset, int64_t* el
 int hadpsgd_padded_len(hadpsgd_handle h, int64_t* P_padded);
 
 /* Synchronises the stream and copies the diagnostics of the most recent step THAT COMPUTED THEM to the
- * host (host_out->step_k says which).                                                               */
+ * host (host_out->step_k says which).
+ * Sharing the device: the cross-block sum of a5 is finished by the LAST blocks of the step's grid, which
+ * wait (bounded spin, no fence, no atomics) for partial sums of blocks with lower ids.  On an idle device
+ * the whole grid is resident and nothing waits for long.  When the SMs are shared -- several handles on
+ * several streams, two processes on one GPU, another library's persistent kernel -- progress relies on
+ * the GPU starting the blocks of a grid in block-id order (true of every NVIDIA GPU to date, not a CUDA
+ * guarantee); supported and tested: up to 4 handles stepping concurrently on their own streams.  If a
+ * collector ever gives up (about a minute), the diagnostics of that step are NaN, the step's w and v are
+ * unaffected, and the next hadpsgd_diagnostics() returns HADPSGD_DIAG_TIMEOUT once instead of data.   */
 int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out);
 /* Switch a5 off / on for the steps that follow (default: on, unless created with HADPSGD_NO_DIAG, which
  * cannot be switched on).  A caller that looks at the diagnostics every N steps only pays for them
  * there: for a small problem their final cross-block reduction is most of a step.
- * Results (w, v) do not depend on it.  Host-only state: no stream work.                               */
+ * Results (w, v) do not depend on it.  Host-only state: no stream work.
+ * HADPSGD_PEER: pend_wsq / pend_gap of a pending mix are delivered by the launch that RESOLVES it (the
+ * next step or hadpsgd_peer_flush); if diagnostics are off for that launch they are never delivered --
+ * keep them on for the step after one whose pend_* you want.                                          */
 int hadpsgd_set_diagnostics(hadpsgd_handle h, int enable);
 
 /* Consensus distance D = sum_i sum_s (w_s[i] - mean_s w_.[i])^2 of the current weights

@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 F32, BF16 = 0, 1
-OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_DEVICE = 0, -1, -2, -3, -4
+OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_DEVICE, DIAG_TIMEOUT = 0, -1, -2, -3, -4, -5
 DETERMINISTIC, NO_MIX, NO_DIAG, EQ7_LITERAL, SHARE_PAIR_WEIGHTS, PEER = 1, 2, 4, 8, 16, 32
 SEG_ALIGN_ELEMS = 64
 MAX_S = 512

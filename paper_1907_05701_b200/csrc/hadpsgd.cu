@@ -47,6 +47,7 @@ struct hadpsgd_ctx {
     // scratch of the step calls: sized by the first step, reused afterwards (no host allocation per step)
     std::vector<int32_t> partner, new_slot, new_pending;
     std::vector<SlotCopy> copies;
+    std::vector<double> diag_host;      // hadpsgd_diagnostics: landing buffer of the device results
     std::vector<WorkItem> part[2][2];   // peer mode: [pairs | singles][plain | pending]
     StepPlan plan;
     // super-learner partition (HADPSGD_PEER)
@@ -129,6 +130,7 @@ int launch_chunk(hadpsgd_ctx* h, const WorkItem* items, int n_items, int mode, i
     a.reverse = h->walk_reverse ? 1 : 0;
     a.S = h->L.S;
     a.partials = h->d_partials; a.diag = h->d_diag;
+    a.timeout_flag = reinterpret_cast<unsigned int*>(h->d_diag + kDiagArrays * h->L.S);   // first spare word behind the results
     if (++h->diag_tag == 0) h->diag_tag = 1;   // a tag is never 0 (zero = empty slot)
     a.tag = h->diag_tag;
     for (int j = 0; j < n_items; ++j) {
@@ -233,9 +235,8 @@ int step_range(hadpsgd_ctx* h, const StepPlan& sp, float lr, float mu, int64_t e
     // loads per member, more registers).  A pair without one reads and writes its members' main
     // buffers -- exactly the kOwn pair kernel -- and a single without one (unmixed, or publishing u for
     // a partner in another arena) is the ordinary kSingle kernel, which addresses weights through the
-    // item's buffer indices anyway.  The plain kernels do not know pend_wsq / pend_gap: clear them.
-    if (!(h->flags & HADPSGD_NO_DIAG) && h->diag_on && !accumulate)
-        CUDA_TRY(h, cudaMemsetAsync(h->d_diag + 3 * h->L.S, 0, sizeof(double) * 2 * h->L.S, h->stream));
+    // item's buffer indices anyway.  Each kernel writes pend_wsq / pend_gap of its own members (the plain
+    // ones write 0), so the up to four launches of a step follow one another with nothing in between.
     for (auto& row : h->part) for (auto& v : row) v.clear();   // [pairs | singles][plain | pending]
     for (const WorkItem& it : sp.pairs) h->part[0][(it.b_s || it.b_p) ? 1 : 0].push_back(it);
     for (const WorkItem& it : sp.singles) h->part[1][it.b_s ? 1 : 0].push_back(it);
@@ -550,9 +551,18 @@ extern "C" int hadpsgd_diagnostics(hadpsgd_handle h, hadpsgd_diag* host_out) {
     if (h->flags & HADPSGD_NO_DIAG) { h->err = "handle was created with HADPSGD_NO_DIAG"; return HADPSGD_INVALID_ARG; }
     DeviceGuard guard(h->device);
     const int S = h->L.S;
-    std::vector<double> tmp(kDiagArrays * S);
-    CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * kDiagArrays * S, cudaMemcpyDeviceToHost, h->stream));
+    std::vector<double>& tmp = h->diag_host;
+    tmp.resize(kDiagArrays * S + 1);              // + the word a collector sets when it gave up waiting
+    CUDA_TRY(h, cudaMemcpyAsync(tmp.data(), h->d_diag, sizeof(double) * (kDiagArrays * S + 1), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    uint32_t timed_out = 0;
+    std::memcpy(&timed_out, &tmp[kDiagArrays * S], sizeof timed_out);
+    if (timed_out) {
+        CUDA_TRY(h, cudaMemsetAsync(h->d_diag + kDiagArrays * S, 0, sizeof(double), h->stream));   // report once
+        h->err = "a step's diagnostics hand-over timed out (the blocks of its grid were not scheduled in order while the "
+                 "device was shared): the diagnostics of that step are NaN; weights and momenta are not affected";
+        return HADPSGD_DIAG_TIMEOUT;
+    }
     host_out->S = S; host_out->n_pairs = h->last_n_pairs; host_out->step_k = h->diag_step_k;
     std::memcpy(host_out->gsq, tmp.data(), sizeof(double) * S);
     std::memcpy(host_out->wsq, tmp.data() + S, sizeof(double) * S);
@@ -731,6 +741,7 @@ extern "C" const char* hadpsgd_error_string(int code) {
         case HADPSGD_OUT_OF_MEMORY: return "out of device memory";
         case HADPSGD_CUDA: return "CUDA error";
         case HADPSGD_UNSUPPORTED_DEVICE: return "unsupported device (sm_100a required)";
+        case HADPSGD_DIAG_TIMEOUT: return "diagnostics hand-over timed out";
         default: return "unknown status";
     }
 }

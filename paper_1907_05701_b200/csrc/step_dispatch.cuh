@@ -6,10 +6,6 @@
 #include "internal.h"
 #include "step_kernel.cuh"
 
-#ifndef HADPSGD_REGCAP
-#define HADPSGD_REGCAP 1   // development switch: 0 builds the fp32 pair kernels without the 128-register cap
-#endif
-
 namespace hadpsgd {
 
 struct LaunchPlan { const void* fn; int threads; int tile_units; int blocks_per_sm; int wmode; };
@@ -45,7 +41,7 @@ LaunchPlan plan_for() {
     // fp32 pair kernels with <= 12 loads per unit need 128-133 registers: capped at 128 so that TWO blocks
     // fit an SM -- not for the persistent grid (one block per SM) but so that the next step's blocks can
     // be resident behind the programmatic dependent launch and a one-wave problem can use 2 x #SMs blocks
-    constexpr int MINB = (HADPSGD_REGCAP && !BF16 && G >= 1 && G <= 4 && U == 1 && MODE != kSingle && WMODE == kOwn && !EMIT && THREADS == 256) ? 2 : 1;
+    constexpr int MINB = (!BF16 && G >= 1 && G <= 4 && U == 1 && MODE != kSingle && WMODE == kOwn && !EMIT && THREADS == 256) ? 2 : 1;
     return {reinterpret_cast<const void*>(&step_kernel<G, BF16, EXACT, DIAG, MODE, EMIT, WMODE, U, THREADS, MINB>),
             THREADS, THREADS * U, BPS, WMODE};
 }

@@ -78,6 +78,7 @@ struct StepArgs {
     int accumulate_diag;  // 0: diag = result ; 1: diag += result (chunked host path)
     int touch_count;      // blocks that work on any one item (host: from n_tiles, grid, walk order)
     int reverse;          // 1: walk the (item, tile) space backwards
+    unsigned int* timeout_flag;   // set to 1 by a collector that gave up waiting (hadpsgd_diagnostics reports it)
     long long keep_from;  // walk position ((item, tile) index; CHAIN: tile index) from which stores stay in L2
     float lr, mu, invG;
     Item items[kInlineItems];
@@ -90,16 +91,10 @@ struct StepArgs {
 // because fewer, longer DRAM bursts are in flight per stream.  (Selecting
 // the policy at run time -- evict_normal when one step's working set fits L2 -- measured no
 // faster at any L2-resident size and 0.4 % slower at full size, so the hint is a literal.)
-#ifndef HADPSGD_LD_L2
-#define HADPSGD_LD_L2 ".L2::evict_first"
-#endif
-#ifndef HADPSGD_ST_L2
-#define HADPSGD_ST_L2 ".L2::evict_first"
-#endif
 struct Raw8 { unsigned u[8]; };
 __device__ __forceinline__ Raw8 ld_stream32(const void* p) {
     Raw8 r;
-    asm volatile("ld.global.L1::no_allocate" HADPSGD_LD_L2 ".v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+    asm volatile("ld.global.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                  : "=r"(r.u[0]), "=r"(r.u[1]), "=r"(r.u[2]), "=r"(r.u[3]), "=r"(r.u[4]), "=r"(r.u[5]), "=r"(r.u[6]), "=r"(r.u[7])
                  : "l"(p));
     return r;
@@ -115,7 +110,7 @@ __device__ __forceinline__ void st_stream32(void* p, const Raw8& r, bool keep) {
                      :: "l"(p), "r"(r.u[0]), "r"(r.u[1]), "r"(r.u[2]), "r"(r.u[3]), "r"(r.u[4]), "r"(r.u[5]), "r"(r.u[6]), "r"(r.u[7])
                      : "memory");
     else
-        asm volatile("st.global.L1::no_allocate" HADPSGD_ST_L2 ".v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+        asm volatile("st.global.L1::no_allocate.L2::evict_first.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                      :: "l"(p), "r"(r.u[0]), "r"(r.u[1]), "r"(r.u[2]), "r"(r.u[3]), "r"(r.u[4]), "r"(r.u[5]), "r"(r.u[6]), "r"(r.u[7])
                      : "memory");
 }
@@ -306,12 +301,19 @@ __device__ __forceinline__ void clear_tagged(TaggedDouble* p) {
     asm volatile("st.volatile.global.v2.u64 [%0], {%1,%1};" :: "l"(p), "l"(0ull) : "memory");
 }
 // Value of a partial already loaded once (t); re-polls until both words carry `tag`.  The writer is a
-// block of the same grid that is resident or finished, so the wait is short; a bounded spin turns
-// a protocol error into NaN diagnostics instead of a hung GPU.
-__device__ __forceinline__ double wait_tagged(const TaggedDouble* p, TaggedDouble t, unsigned tag) {
+// block of the same grid with a LOWER block id (see the collector below), i.e. one that was handed to
+// an SM before this block was: it is running or finished, so the wait is short.  That rests on the
+// hardware dispatching the blocks of a grid in block-id order, which every NVIDIA GPU so far does but
+// CUDA does not promise; should it ever not hold while the SMs are shared with other work, a bounded
+// spin turns the stall into NaN diagnostics PLUS a flag that hadpsgd_diagnostics reports as
+// HADPSGD_DIAG_TIMEOUT, instead of a hung GPU or a silent NaN (w and v never depend on this).
+__device__ __forceinline__ double wait_tagged(const TaggedDouble* p, TaggedDouble t, unsigned tag, unsigned int* timeout_flag) {
     unsigned spins = 0;
     while (static_cast<unsigned>(t.lo >> 32) != tag || static_cast<unsigned>(t.hi >> 32) != tag) {
-        if (++spins > (1u << 26)) return __longlong_as_double(0x7ff8000000000000ll);   // about a minute
+        if (++spins > (1u << 26)) {   // about a minute
+            *reinterpret_cast<volatile unsigned int*>(timeout_flag) = 1u;
+            return __longlong_as_double(0x7ff8000000000000ll);
+        }
         if (spins > 16) __nanosleep(spins > 4096 ? 512 : 32);
         t = ld_tagged(p);
     }
@@ -620,6 +622,13 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             } else if (k == 4) {
                 put(gap + s, 0.0);
             }
+            if constexpr (!PEER) {
+                // a member that resolves no pending mix owes nothing from the step before: its pend_wsq /
+                // pend_gap read 0 (every member is in exactly one item of a step, so a step rewrites all S)
+                double* pws = a.diag + 3 * S; double* pgp = a.diag + 4 * S;
+                if (k == 2) { put(pws + s, 0.0); put(pgp + s, 0.0); }
+                if (PAIRED && k == 3) { put(pws + p, 0.0); put(pgp + p, 0.0); }
+            }
             if constexpr (PEER) {
                 double* pws = a.diag + 3 * S; double* pgp = a.diag + 4 * S;
                 if (k == 5) put(pws + s, sum);
@@ -649,9 +658,13 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
             st_tagged(a.partials + static_cast<size_t>(blockIdx.x) * R + row, tot, a.tag);
         }
         // Item j is COLLECTED by block grid-1 - (j mod grid): the blocks with the highest ids, which are
-        // dispatched last and have the fewest tiles.  Every other block is done here.  (The whole grid is
-        // resident at once -- the host sizes it so -- hence a collector never waits for a block that
-        // cannot run.)  Item j was worked on by exactly touch_count blocks: the i-th of them (in tile
+        // dispatched last and have the fewest tiles.  Every other block is done here.  Forward progress:
+        // a collector only waits for blocks with LOWER ids than its own (or itself), and blocks are handed
+        // to SMs in block-id order, so by the time a collector runs every block it waits for is running or
+        // done.  When the device is otherwise idle the whole grid is resident at once (the host sizes it
+        // to this kernel's occupancy) and the order does not even matter; when the SMs are shared (other
+        // handles on other streams, another process, a foreign persistent kernel) in-order dispatch is
+        // what is relied on -- see wait_tagged for what happens if it failed.  Item j was worked on by exactly touch_count blocks: the i-th of them (in tile
         // order) is block (j * n_tiles + i) mod grid in the item-major walk, (j + i * n_work) mod grid in the
         // tile-major walk, block i in the CHAIN walk.  One warp per quantity: lane l polls contributors l,
         // l+32, ... (eight independent loads at a time), adds them in that order, the lanes combine in a
@@ -682,7 +695,7 @@ __global__ void __launch_bounds__(THREADS, MINB) step_kernel(const __grid_consta
 #pragma unroll
                     for (int m = 0; m < 8; ++m) {
                         if (i0 + 32 * m < a.touch_count) {
-                            sum += wait_tagged(src[m], t[m], a.tag);
+                            sum += wait_tagged(src[m], t[m], a.tag, a.timeout_flag);
                             clear_tagged(src[m]);
                         }
                     }

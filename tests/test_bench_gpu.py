@@ -31,7 +31,7 @@ def test_gpu_arm_line_has_the_contract_keys():
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["frac"] == pytest.approx(r["achieved"] / r["peak"])
     assert r["algorithmic_bytes_per_launch"] == 2 * 1_000_000 * 24
     assert r["traffic"] is None and r["traffic_source"]                    # no ncu capture of this workload: never a guess
-    assert r["ceiling"]["read_gbs"] > 1000 and r["ceiling"]["write_gbs"] > 1000
+    assert r["reference_mix"]["read_gbs"] > 1000 and r["reference_mix"]["write_gbs"] > 1000
     e = d["e2e"]
     assert e["h2d_bytes_per_step"] == 2 * 2 * 1_000_000 * 4 and e["d2h_bytes_per_step"] > 0 and 0 < e["value"] < d["value"]
     c = d["cpu_baseline"]

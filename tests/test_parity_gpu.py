@@ -1129,27 +1129,35 @@ def test_config2_swb2000_whole_buffer_every_element(H, oracle_mod, torch_cuda):
     seeded generator (bit-compared with the numpy one in test_device_generator_matches_host),
     generated per window and copied down -- 100 GB of numpy hashing would take minutes."""
     import os
+    import threading
     from concurrent.futures import ThreadPoolExecutor
     torch = torch_cuda
+    diag_lock = threading.Lock()
     from fixtures import device, generator as gen, problem, shapes
     cfg = shapes.CONFIGS["swb2000"]
     S, G, P, steps, seed = cfg["S"], cfg["G"], int(sum(cfg["seg_len"])), 2, 4242
     h = H.Hadpsgd(S, G, cfg["seg_len"], H.F32, H.DETERMINISTIC)
     assert h.P_padded == P
     problem.fill_weights(h, seed)
+    gdiag = []
     for k in range(steps):
         problem.fill_grads(h, seed, k)
         h.hadpsgd_step(LR, MU, k)
+        gdiag.append(h.hadpsgd_diagnostics())
     torch.cuda.synchronize()
     assert h.hadpsgd_launch_count() == steps
     n_threads = os.cpu_count() or 1
     W = 1 << 20
     compared = {"w": 0, "v": 0}
+    odiag = [{q: np.zeros(S) for q in ("gsq", "wsq", "gap")} for _ in range(steps)]   # the oracle's a5, summed over windows
 
     def check(lo, hi, w0, grads, gw, gv):
         ow, ov = w0, np.zeros((S, hi - lo), np.float32)
         for k in range(steps):
-            oracle_mod.step(grads[k], ow, ov, LR, MU, k)
+            d = oracle_mod.step(grads[k], ow, ov, LR, MU, k, diag=True)
+            with diag_lock:
+                for q in odiag[k]:
+                    odiag[k][q] += d[q]
         bad_w, bad_v = int(np.sum(bits(gw) != bits(ow))), int(np.sum(bits(gv) != bits(ov)))
         return lo, hi, bad_w, bad_v
 
@@ -1180,6 +1188,9 @@ def test_config2_swb2000_whole_buffer_every_element(H, oracle_mod, torch_cuda):
             assert bw == 0 and bv == 0, (lo_, hi_, bw, bv)
             compared["w"] += S * (hi_ - lo_); compared["v"] += S * (hi_ - lo_)
     assert compared["w"] == S * P and compared["v"] == S * P       # every element of every buffer
+    for k in range(steps):          # a5 at full size against the oracle's double accumulators (Q16: relative 1e-4)
+        for q in ("gsq", "wsq", "gap"):
+            assert np.allclose(gdiag[k][q], odiag[k][q], rtol=1e-4, atol=0), (k, q, gdiag[k][q], odiag[k][q])
     h.close()
     del dev_w0, dev_g
     torch.cuda.empty_cache()
