@@ -288,12 +288,22 @@ const char* hadpsgd_consensus_noalloc_error(void);
  * reading the partner's stage buffer through a peer pointer inside the same fused pass -- 4 B per
  * parameter per pending member cross the link per step, and no kernel ever waits on another one.
  * Same arithmetic as the single-arena step: bit-exact in DETERMINISTIC mode.
- *   Contract: (1) every rank makes the same sequence of step calls (like a collective); each call
- * advances the handle's epoch; (2) EPOCH BARRIER -- a rank must not enqueue epoch e+1 before every
- * rank's epoch-e kernel has completed: one stream when the handles share a device, else a
- * stream-ordered barrier between steps (e.g. an NCCL all-reduce of one element on the handle's
- * stream); (3) hadpsgd_weights(h, s) is INVALID_ARG while s is pending -- call hadpsgd_peer_flush()
- * (after the epoch barrier) to materialise every pending mix into the main weight buffers.       */
+ *   Contract: (1) every rank makes the same sequence of step calls with the same matchings (like a
+ * collective); each call advances the handle's epoch; (2) hadpsgd_weights(h, s) is INVALID_ARG while s
+ * is pending -- call hadpsgd_peer_flush() to materialise every pending mix into the main weight buffers.
+ *   Ordering between ranks is the LIBRARY's business (there is no epoch barrier for the caller to
+ * provide, and no global one anywhere -- PAPER.md:62 "averages its weights with its neighbor", :66 "removes
+ * the global barrier"): every handle owns a 32-bit epoch word behind its stage buffers, writes e + 1 there
+ * with a stream memory operation after the last launch of its step e, and before the first launch of a
+ * step (or flush) makes its stream wait on the words of exactly the ranks whose stage buffers it is about
+ * to read, or which must first have read what it is about to overwrite -- its partners of the last two
+ * steps, two ranks in the ring.  The waits are stream operations (cuStreamWaitValue32): no kernel spins
+ * and no SM is held, so ranks may share one GPU, run on streams of their own, or live in different
+ * processes; a rank that runs ahead simply blocks in its stream until its neighbour has caught up.
+ * Consequences: handles that share ONE stream must be stepped epoch by epoch (all handles' step e before
+ * any handle's step e + 1 -- the other order waits for a write queued behind itself); a step sequence
+ * captured into a CUDA graph replays fixed epoch values and is therefore not ordered by the handshake.
+ * hadpsgd_peer_init synchronises the stream once (the word must be zero before peers learn of it).    */
 
 /* rank_begin: host [world+1], increasing, rank_begin[0] = 0, rank_begin[world] = S_global <= HADPSGD_MAX_S. */
 int hadpsgd_peer_init(hadpsgd_handle h, int rank, int world, const int32_t* rank_begin);
@@ -317,8 +327,10 @@ int hadpsgd_peer_ipc_export(hadpsgd_handle h, void* ipc_handle_out, uint64_t* st
  * previous mapping and opens the new one; hadpsgd_destroy() closes what is left.                    */
 int hadpsgd_peer_ipc_attach(hadpsgd_handle h, int r, const void* ipc_handle, uint64_t stage_offset);
 /* Materialise every pending mix: w_s = 1/2 (u_own + u_partner) into the main weight buffer (one small
- * kernel on the stream; asynchronous), delivering pend_wsq / pend_gap.  Call after the epoch barrier.
- * Not a step: the epoch does not advance, ranks need not call it together.                          */
+ * kernel on the stream; asynchronous), delivering pend_wsq / pend_gap.  It first waits, on the stream,
+ * for the partners' publishing step (epoch handshake).  Not a step: the epoch does not advance, ranks
+ * need not call it together.  A rank must not destroy its handle (or free its arena) while a partner
+ * may still flush or step against it: agree on teardown outside this library.                      */
 int hadpsgd_peer_flush(hadpsgd_handle h);
 /* The peer plan of one step as a pure host function (no GPU): see csrc/scheduler.cpp.  pending: in/out
  * [S_local] (global partner index or -1); outputs [S_local]: kind (0 pair member, 1 unmixed,

@@ -48,6 +48,10 @@ int compute_layout(int S, int G, const int64_t* seg_len, int n_seg, hadpsgd_dtyp
     L.w_off = cur;
     L.stage_off = cur + static_cast<size_t>(S) * L.w_stride_bytes();
     cur = round_up(cur + static_cast<size_t>(S) * (L.peer_stage ? 3 : 1) * L.w_stride_bytes(), kRegionAlign);
+    if (L.peer_stage) {   // the epoch word of the neighbour handshake, directly behind the stage buffers (a buffer is a
+        L.epoch_off = L.stage_off + static_cast<size_t>(2) * S * L.w_stride_bytes();   // multiple of 256 B, so no gap)
+        cur = L.epoch_off + kRegionAlign;
+    }
     L.v_off = cur; cur = round_up(cur + static_cast<size_t>(S) * L.w_stride_bytes(), kRegionAlign);
     L.g_off = cur; cur = round_up(cur + static_cast<size_t>(S) * G * L.g_stride_bytes(), kRegionAlign);
     L.wb_off = cur;

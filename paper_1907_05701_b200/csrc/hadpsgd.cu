@@ -58,6 +58,9 @@ struct hadpsgd_ctx {
     std::vector<int32_t> pending;              // [S] global partner whose stage completes w_s, or -1
     uint64_t epoch = 0;
     const float** d_peer = nullptr;            // device table [2][S_global]
+    // neighbour-only epoch handshake: war_until[parity][q] = value rank q's epoch word must have reached before this
+    // handle overwrites its stage buffers of that parity again (0: no reader outstanding)
+    std::vector<uint32_t> war_until[2], wait_value;
     std::vector<void*> ipc_mapped;             // [world] the cudaIpcOpenMemHandle mapping of rank r (nullptr: none); closed on re-attach and at destroy
     std::string err;
 };
@@ -285,6 +288,92 @@ int upload_peer_table(hadpsgd_ctx* h) {
     return HADPSGD_OK;
 }
 
+// ---- neighbour-only epoch handshake (HADPSGD_PEER) -------------------------------------------------
+// Every handle owns one 32-bit EPOCH WORD behind its stage buffers (Layout::epoch_off; inside the arena,
+// so it is reachable wherever the stage region is: same device, peer device, CUDA IPC mapping).  After the
+// last launch of its step number e (e = 0, 1, ...) a handle writes e + 1 there with a stream memory
+// operation; before the first launch of a step it makes its stream wait (>=) on the words of exactly the
+// ranks it exchanges stage buffers with:
+//   RAW  a member whose mix with a partner in rank q is pending reads q's stage buffer of step e - 1:
+//        wait word_q >= e.  (hadpsgd_peer_flush: the same.)
+//   WAR  a handle that published u for a partner in rank q at step e0 must not overwrite that stage
+//        parity (step e0 + 2 at the earliest) before q has read it, which q does in its step e0 + 1 (or
+//        in a flush enqueued before that step): wait word_q >= e0 + 2.
+// These are stream operations (cuStreamWaitValue32 / cuStreamWriteValue32): no kernel spins, nothing
+// occupies an SM while waiting, so ranks that share one GPU cannot starve each other, and no rank ever
+// waits for a rank that is not its partner -- there is no global barrier.
+using stream_memop_fn = int (*)(cudaStream_t, unsigned long long, uint32_t, unsigned int);
+struct StreamMemOps { stream_memop_fn write = nullptr, wait = nullptr; };
+
+int get_stream_memops(hadpsgd_ctx* h, StreamMemOps* out) {
+    static StreamMemOps ops;      // resolved once per process (benign race: both threads store the same pointers)
+    if (!ops.write || !ops.wait) {
+        void* fw = nullptr; void* fq = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        CUDA_TRY(h, cudaGetDriverEntryPoint("cuStreamWriteValue32", &fw, cudaEnableDefault, &qr));
+        if (!fw || qr != cudaDriverEntryPointSuccess) { h->err = "cuStreamWriteValue32 is unavailable"; return HADPSGD_CUDA; }
+        CUDA_TRY(h, cudaGetDriverEntryPoint("cuStreamWaitValue32", &fq, cudaEnableDefault, &qr));
+        if (!fq || qr != cudaDriverEntryPointSuccess) { h->err = "cuStreamWaitValue32 is unavailable"; return HADPSGD_CUDA; }
+        ops.write = reinterpret_cast<stream_memop_fn>(fw);
+        ops.wait = reinterpret_cast<stream_memop_fn>(fq);
+    }
+    *out = ops;
+    return HADPSGD_OK;
+}
+
+int owner_rank(const hadpsgd_ctx* h, int global_member) {
+    int r = 0;
+    while (r + 1 < h->world && global_member >= h->rank_begin[r + 1]) ++r;
+    return r;
+}
+
+// Device address of rank r's epoch word, from the stage region this process attached for it.
+unsigned long long epoch_word_of(const hadpsgd_ctx* h, int r) {
+    const size_t n = static_cast<size_t>(h->rank_begin[r + 1] - h->rank_begin[r]);
+    return reinterpret_cast<unsigned long long>(h->stage_of_rank[r]) + 2 * n * h->L.w_stride_bytes();
+}
+
+// Enqueues the waits a step (for_step) or a flush needs before its first launch.
+int epoch_wait(hadpsgd_ctx* h, bool for_step) {
+    if (h->world < 2) return HADPSGD_OK;
+    const uint32_t e = static_cast<uint32_t>(h->epoch);
+    std::vector<uint32_t>& need = h->wait_value;
+    need.assign(h->world, 0);
+    for (int s = 0; s < h->L.S; ++s)
+        if (h->pending[s] >= 0) need[owner_rank(h, h->pending[s])] = e;                       // RAW
+    if (for_step) {
+        std::vector<uint32_t>& war = h->war_until[e & 1];
+        for (int q = 0; q < h->world; ++q) { if (war[q] > need[q]) need[q] = war[q]; war[q] = 0; }   // WAR
+    }
+    StreamMemOps ops;
+    for (int q = 0; q < h->world; ++q) {
+        if (!need[q] || q == h->rank) continue;
+        if (!ops.wait) { const int rc = get_stream_memops(h, &ops); if (rc != HADPSGD_OK) return rc; }
+        if (ops.wait(h->stream, epoch_word_of(h, q), need[q], 0u /* CU_STREAM_WAIT_VALUE_GEQ */) != 0) {
+            h->err = "cuStreamWaitValue32 on the epoch word of rank " + std::to_string(q) + " failed";
+            return HADPSGD_CUDA;
+        }
+    }
+    return HADPSGD_OK;
+}
+
+// After the last launch of step `epoch`: publish epoch + 1, and remember who must have read what this
+// step published before its stage parity is written again.
+int epoch_signal(hadpsgd_ctx* h, const std::vector<int32_t>& new_pending) {
+    if (h->world < 2) return HADPSGD_OK;
+    const uint32_t e = static_cast<uint32_t>(h->epoch);
+    StreamMemOps ops;
+    const int rc = get_stream_memops(h, &ops);
+    if (rc != HADPSGD_OK) return rc;
+    if (ops.write(h->stream, reinterpret_cast<unsigned long long>(h->arena + h->L.epoch_off), e + 1u, 0u) != 0) {
+        h->err = "cuStreamWriteValue32 on the epoch word failed";
+        return HADPSGD_CUDA;
+    }
+    for (int s = 0; s < h->L.S; ++s)
+        if (new_pending[s] >= 0) h->war_until[e & 1][owner_rank(h, new_pending[s])] = e + 2u;
+    return HADPSGD_OK;
+}
+
 // Matching -> work items with weight buffers.  Nothing of the handle's state is committed here: the
 // caller commits `new_slot` / `new_pending` once every launch of the step has been enqueued.
 int plan_and_prepare(hadpsgd_ctx* h, const int32_t* partner, StepPlan* sp, std::vector<int32_t>* new_slot,
@@ -437,8 +526,10 @@ extern "C" int hadpsgd_step_matching(hadpsgd_handle h, float lr, float momentum,
     if (rc != HADPSGD_OK) return rc;
     rc = plan_and_prepare(h, h->partner.data(), &h->plan, &h->new_slot, &h->new_pending);
     if (rc != HADPSGD_OK) return rc;
+    if (is_peer(h)) { rc = epoch_wait(h, true); if (rc != HADPSGD_OK) return rc; }   // neighbours only, on the stream
     rc = step_range(h, h->plan, lr, momentum, 0, h->L.P_padded, false);
     if (rc != HADPSGD_OK) return rc;
+    if (is_peer(h)) { rc = epoch_signal(h, h->new_pending); if (rc != HADPSGD_OK) return rc; }
     commit_plan(h, h->plan, h->new_slot, h->new_pending, step_k);   // only now: every launch is enqueued
     return HADPSGD_OK;
 }
@@ -620,6 +711,11 @@ extern "C" int hadpsgd_peer_init(hadpsgd_handle h, int rank, int world, const in
     }
     for (void* p : h->ipc_mapped) if (p) cudaIpcCloseMemHandle(p);   // a repeated init (before the first step) starts over
     h->ipc_mapped.assign(world, nullptr);
+    h->war_until[0].assign(world, 0);
+    h->war_until[1].assign(world, 0);
+    // the epoch word (zeroed with the arena at create, on the stream) must be zero before any peer can learn
+    // its address, which it does through calls that follow this one
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->rank = rank; h->world = world; h->S_global = rank_begin[world];
     h->rank_begin.assign(rank_begin, rank_begin + world + 1);
     h->stage_of_rank.assign(world, nullptr);
@@ -704,6 +800,8 @@ extern "C" int hadpsgd_peer_flush(hadpsgd_handle h) {
         if (h->pending[s] >= 0) { members.push_back(s); members.push_back(rd * h->S_global + h->pending[s]); }
     if (members.empty()) return HADPSGD_OK;
     int rc = upload_peer_table(h);
+    if (rc != HADPSGD_OK) return rc;
+    rc = epoch_wait(h, false);          // the partners' publishing step must have completed
     if (rc != HADPSGD_OK) return rc;
     cudaError_t e = cudaSuccess;
     const float* a_stage = reinterpret_cast<const float*>(h->arena + h->L.stage_off) + static_cast<size_t>(rd) * h->L.S * h->L.P_padded;

@@ -23,6 +23,8 @@ struct Layout {
     std::vector<int64_t> seg_len, seg_offset;
     size_t w_off = 0, v_off = 0, g_off = 0;  // byte offsets inside the arena
     size_t stage_off = 0;                    // = w_off + S weight buffers: [2][S] stage buffers (peer_stage only)
+    size_t epoch_off = 0;                    // = stage_off + 2 S buffers: this handle's 32-bit epoch word on a 256 B line of
+                                             // its own (peer_stage only); peers find it from the stage pointer they attached
     size_t wb_off = 0;                       // bf16 working copies (S x P_padded x 2 B), if any
     size_t aux_off = 0, aux_bytes = 0;       // diagnostics scratch: tagged partials | plain scratch | results
     size_t partials_bytes = 0, scratch_bytes = 0;

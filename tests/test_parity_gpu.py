@@ -464,7 +464,10 @@ def test_peer_errors(H):
 
 def _ipc_worker(rank, world, port, out_dir):
     """One process per rank, BOTH ON GPU 0: stage regions are exchanged as CUDA IPC handles (gloo carries
-    the 64 bytes), the epoch barrier is synchronize + a gloo barrier.  No kernel waits on another."""
+    the 64 bytes).  Between steps there is NO synchronize and NO barrier: the library's neighbour-only epoch
+    handshake (stream waits on the partner's epoch word, through the IPC mapping) orders the two
+    processes; rank 1 is delayed on purpose so that rank 0 runs ahead and must block.  No kernel waits on
+    another."""
     import os
     import torch
     import torch.distributed as dist
@@ -494,9 +497,9 @@ def _ipc_worker(rank, world, port, out_dir):
             for s in range(4):
                 for g in range(G):
                     device.fill(h.hadpsgd_grads(s, g)[:P], gen.stream_key(seed, gen.STREAM_GRAD, k, lo + s, g), "normal", 1e-3)
-            h.hadpsgd_step(0.1, 0.9, k)
-            torch.cuda.synchronize()
-            dist.barrier()                              # epoch barrier
+            if rank == 1 and k in (1, 3):
+                torch.cuda._sleep(400_000_000)          # ~0.2 s: the other process gets two steps ahead of this one
+            h.hadpsgd_step(0.1, 0.9, k)                 # no synchronize, no barrier: the epoch handshake orders the ranks
         h.hadpsgd_peer_flush()
         torch.cuda.synchronize()
         dist.barrier()                                  # nobody tears its stage region down before all have read it

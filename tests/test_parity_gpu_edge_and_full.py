@@ -312,3 +312,64 @@ def test_every_element_swb2000_default_mode(H, oracle_mod, torch_cuda):
     """Headline shape in DEFAULT mode (FMA contraction allowed): every element within the stated
     tolerance 1e-6 + 1e-5 |x| (north_star), diagnostics at rel 1e-4 -- the kernel bench.py times."""
     every_element(H, oracle_mod, torch_cuda, "swb2000", exact=False)
+
+
+# ------------------------------------------------------------------ neighbour-only epoch handshake (row f4)
+
+@pytest.mark.parametrize("delay_rank", [None, 0, 2])
+def test_peer_ranks_on_their_own_streams_are_ordered_by_the_epoch_handshake(H, oracle_mod, torch_cuda, delay_rank):
+    """Four HADPSGD_PEER handles ("ranks") on ONE GPU, each on a stream of its own, stepped without any
+    host synchronisation or shared stream in between: what orders rank r's step e + 1 behind its partners'
+    step e is the library's neighbour-only handshake (no global barrier).  Ring steps,
+    then custom matchings with far partners and unmixed members; bit-exact against the oracle.  With one
+    rank delayed by a ~1 s spin on its stream, its partner is shown to be BLOCKED (stream not idle) while
+    the sleeper runs, and the results are still exact -- without the waits the partner would have read a
+    stage buffer that had not been written yet."""
+    torch = torch_cuda
+    from fixtures import device, generator as gen, problem
+    rank_begin, G, P, seed = [0, 2, 4, 6, 8], 2, 300_007, 907
+    R, S = len(rank_begin) - 1, rank_begin[-1]
+    streams = [torch.cuda.Stream() for _ in range(R)]
+    hs = [H.Hadpsgd(2, G, [P], H.F32, H.PEER | H.DETERMINISTIC, stream=streams[r]) for r in range(R)]
+    for r, h in enumerate(hs):
+        h.hadpsgd_peer_init(r, R, rank_begin)
+    for r, h in enumerate(hs):
+        for q, other in enumerate(hs):
+            if q != r:
+                h.hadpsgd_peer_attach(q, other.hadpsgd_peer_stage())
+    for sg in range(S):                       # ONE set of gradients, reused by every step: nothing to refill in between
+        h, s = hs[sg // 2], sg % 2
+        device.fill(h.hadpsgd_weights(s)[:P], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, sg, 0), "normal", 0.05)
+        for g in range(G):
+            device.fill(h.hadpsgd_grads(s, g)[:P], gen.stream_key(seed, gen.STREAM_GRAD, 0, sg, g), "normal", 1e-3)
+    torch.cuda.synchronize()
+    ring = lambda k: [(s + 1 if s % 2 == 0 else s - 1) if k % 2 == 0 else ((s + 1) % S if s % 2 == 1 else (s - 1) % S) for s in range(S)]
+    matchings = [None] * 6 + [[7, 6, 5, 4, 3, 2, 1, 0], [1, 0, 3, 2, 5, 4, 7, 6], [0, 2, 1, 4, 3, 6, 5, 7],
+                              [4, 5, 6, 7, 0, 1, 2, 3], None, None]
+    for k, m in enumerate(matchings):                      # enqueue everything; the host never waits for the GPU
+        if k == 2 and delay_rank is not None:              # (the first step of a handle uploads its peer table and
+            with torch.cuda.stream(streams[delay_rank]):   # synchronises its stream once, so the delay comes later)
+                torch.cuda._sleep(2_000_000_000)           # about a second
+        for h in hs:
+            if m is None:
+                h.hadpsgd_step(LR, MU, k)
+            else:
+                h.hadpsgd_step_matching(LR, MU, k, m)
+    if delay_rank is not None:
+        # step 1 published u across the arenas ((1,2) (3,4) (5,6) (7,0)) into stage parity 1 and step 2
+        # resolves it; step 3 publishes into parity 1 again, so the sleeper's ring neighbours are stuck in
+        # front of their step 3 until the sleeper has finished ITS step 2 (the reader of what they overwrite)
+        assert not streams[delay_rank].query()
+        assert not streams[(delay_rank + 1) % R].query() and not streams[(delay_rank - 1) % R].query()
+    for h in hs:
+        h.hadpsgd_peer_flush()
+    torch.cuda.synchronize()
+    og = problem.host_grads(seed, 0, S, G, 0, P)
+    ow, ov = problem.host_weights(seed, S, 0, P), np.zeros((S, P), np.float32)
+    for k, m in enumerate(matchings):
+        oracle_mod.step(og, ow, ov, LR, MU, k, partner=m if m is not None else ring(k))
+    gw = np.stack([hs[sg // 2].hadpsgd_weights(sg % 2)[:P].cpu().numpy() for sg in range(S)])
+    gv = np.stack([hs[sg // 2].hadpsgd_momentum(sg % 2)[:P].cpu().numpy() for sg in range(S)])
+    assert np.array_equal(bits(gw), bits(ow)) and np.array_equal(bits(gv), bits(ov))
+    for h in hs:
+        h.close()
