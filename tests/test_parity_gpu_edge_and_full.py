@@ -373,3 +373,110 @@ def test_peer_ranks_on_their_own_streams_are_ordered_by_the_epoch_handshake(H, o
     assert np.array_equal(bits(gw), bits(ow)) and np.array_equal(bits(gv), bits(ov))
     for h in hs:
         h.close()
+
+
+def test_every_element_peer_group_of_8_at_full_size(H, oracle_mod, torch_cuda):
+    """The super-learner partition at the headline size, in the shape `bench.py --emulate-ranks 8` times: 8
+    HADPSGD_PEER arenas of 2 x 145,145,344 parameters on one GPU (74 GB), ring steps 0..3 (inside the
+    arenas, across them, resolve inside the fused kernel, across them again) and a final flush.  EVERY
+    element of all 16 weight and momentum buffers against the oracle, bit for bit, and the a5 sums of every
+    step against the oracle's double accumulators: gsq at once; wsq / gap at once for members whose mix
+    finished inside the step, and as pend_wsq / pend_gap of the NEXT step (or of the flush) for members
+    whose partner lives in another arena.  This is the kPeer kernel on a grid that is busy for thousands of
+    tiles per block, which the small peer tests never reach."""
+    torch = torch_cuda
+    from fixtures import device, generator as gen, problem, shapes
+    cfg = shapes.CONFIGS["swb2000"]
+    S, G, P, R, steps, seed = cfg["S"], cfg["G"], int(sum(cfg["seg_len"])), 8, 4, 5151
+    S_l = S // R
+    rank_begin = [r * S_l for r in range(R + 1)]
+    hs = [H.Hadpsgd(S_l, G, [P], H.F32, H.PEER | H.DETERMINISTIC) for _ in range(R)]
+    for r, h in enumerate(hs):
+        h.hadpsgd_peer_init(r, R, rank_begin)
+    for r, h in enumerate(hs):
+        for q, other in enumerate(hs):
+            if q != r:
+                h.hadpsgd_peer_attach(q, other.hadpsgd_peer_stage())
+    where = lambda sg: (hs[sg // S_l], sg % S_l)
+    for sg in range(S):
+        h, s = where(sg)
+        device.fill(h.hadpsgd_weights(s), gen.stream_key(seed, gen.STREAM_WEIGHT, 0, sg, 0), "normal", 0.05)
+    gdiag = []                                             # [step][rank] -> diagnostics dict
+    for k in range(steps):
+        for sg in range(S):
+            h, s = where(sg)
+            for g in range(G):
+                device.fill(h.hadpsgd_grads(s, g), gen.stream_key(seed, gen.STREAM_GRAD, k, sg, g), "normal", 1e-3)
+        for h in hs:                                       # one stream, epoch by epoch
+            h.hadpsgd_step(LR, MU, k)
+        gdiag.append([h.hadpsgd_diagnostics() for h in hs])
+    for h in hs:
+        h.hadpsgd_peer_flush()
+    after_flush = [h.hadpsgd_diagnostics() for h in hs]
+    torch.cuda.synchronize()
+    launches = sum(h.hadpsgd_launch_count() for h in hs)
+    n_threads = os.cpu_count() or 1
+    W = 1 << 20
+    odiag = [{q: np.zeros(S) for q in ("gsq", "wsq", "gap")} for _ in range(steps)]
+    compared = 0
+
+    def check(lo, hi, w0, grads, gw, gv):
+        ow, ov = w0, np.zeros((S, hi - lo), np.float32)
+        ds = [oracle_mod.step(grads[k], ow, ov, LR, MU, k, diag=True) for k in range(steps)]
+        return lo, hi, int(np.sum(bits(gw) != bits(ow))) + int(np.sum(bits(gv) != bits(ov))), ds
+
+    def drain(f):
+        nonlocal compared
+        lo_, hi_, bad, ds = f.result()
+        assert bad == 0, (lo_, hi_, bad)
+        compared += S * (hi_ - lo_)
+        for k in range(steps):
+            for q in ("gsq", "wsq", "gap"):
+                odiag[k][q] += ds[k][q]
+
+    dev_w0 = torch.empty((S, W), dtype=torch.float32, device="cuda")
+    dev_g = torch.empty((steps, S, G, W), dtype=torch.float32, device="cuda")
+    futures = []
+    with ThreadPoolExecutor(max_workers=n_threads) as pool:
+        for lo in range(0, P, W):
+            hi = min(lo + W, P)
+            n = hi - lo
+            for s in range(S):
+                device.fill(dev_w0[s], gen.stream_key(seed, gen.STREAM_WEIGHT, 0, s, 0), "normal", 0.05, elem_offset=lo, n=n)
+                for k in range(steps):
+                    for g in range(G):
+                        device.fill(dev_g[k, s, g], gen.stream_key(seed, gen.STREAM_GRAD, k, s, g), "normal", 1e-3,
+                                    elem_offset=lo, n=n)
+            w0 = np.ascontiguousarray(dev_w0[:, :n].cpu().numpy())
+            grads = [np.ascontiguousarray(dev_g[k, :, :, :n].cpu().numpy()) for k in range(steps)]
+            gw = np.stack([where(sg)[0].hadpsgd_weights(where(sg)[1])[lo:hi].cpu().numpy() for sg in range(S)])
+            gv = np.stack([where(sg)[0].hadpsgd_momentum(where(sg)[1])[lo:hi].cpu().numpy() for sg in range(S)])
+            futures.append(pool.submit(check, lo, hi, w0, grads, gw, gv))
+            while len(futures) > 2 * n_threads:
+                drain(futures.pop(0))
+        for f in futures:
+            drain(f)
+    assert compared == S * P
+    close = lambda a, b: np.allclose(a, b, rtol=1e-4, atol=0)
+    n_pending = 0
+    for k in range(steps):
+        owed_by = gdiag[k + 1] if k + 1 < steps else after_flush        # who delivers what step k left pending
+        for r in range(R):
+            lo, hi = rank_begin[r], rank_begin[r + 1]
+            d = gdiag[k][r]
+            assert close(d["gsq"], odiag[k]["gsq"][lo:hi]), (k, r)
+            pend = d["pending"] == 1
+            n_pending += int(pend.sum())
+            assert close(d["wsq"][~pend], odiag[k]["wsq"][lo:hi][~pend]) and close(d["gap"][~pend], odiag[k]["gap"][lo:hi][~pend]), (k, r)
+            assert close(owed_by[r]["pend_wsq"][pend], odiag[k]["wsq"][lo:hi][pend]), (k, r)
+            assert close(owed_by[r]["pend_gap"][pend], odiag[k]["gap"][lo:hi][pend]), (k, r)
+            assert not owed_by[r]["pend_wsq"][~pend].any() and not owed_by[r]["pend_gap"][~pend].any(), (k, r)
+    assert n_pending == 2 * S                              # steps 1 and 3: every member's ring partner is in another arena
+    assert not any(d["pending"].any() for d in after_flush)
+    # launches: steps 0 and 1 one plain pair / single launch per rank, step 2 one pending-pair launch, step 3
+    # one single launch, then one flush (two kernels, counted once)
+    assert launches == R * (steps + 1), launches
+    for h in hs:
+        h.close()
+    del dev_w0, dev_g
+    torch.cuda.empty_cache()
